@@ -1,0 +1,187 @@
+/*
+ * lbm.h -- C-ABI boundary of the B200-native Shan-Chen multiphase lattice-Boltzmann step.
+ *
+ * What is computed: the per-timestep update of the JAX-LaB paper (arxiv 2506.17713):
+ *   Eq. 1-3   collide (BGK / MRT) + stream
+ *   Eq. 4,10  moments rho^k, j^k per component
+ *   Eq. 5-6   exact-difference forcing, half-force velocity on output
+ *   Eq. 12 pseudopotential psi(rho) from an equation of state
+ *   Eq. 13 Shan-Chen interaction force F_SC, 1 or 2 components
+ *   Eq. 17 improved virtual-density wetting at solid nodes
+ *   no-slip bounce-back, pressure / flux inlet-outlet
+ * on D2Q9 and D3Q19.  Where the paper is silent the readings R1..R17 of DESIGN.md
+ * apply (they restate SURVEY.md section 8(c) G1..G17).
+ *
+ * Conventions
+ *   - All functions are extern "C" and return int: LBM_OK (0) or a negative lbm_status.
+ *     No exceptions, no abort, nothing printed.  lbm_last_error(h) gives a library-owned
+ *     message valid until the next call on h.
+ *   - Every step of the path runs in CUDA kernels for sm_100a.  There is NO CPU fallback:
+ *     without a CUDA device lbm_create fails with LBM_E_CUDA.
+ *   - The library allocates no device memory.  The caller passes ONE device workspace of at
+ *     least lbm_workspace_bytes(cfg) bytes (256-byte aligned) and a cudaStream_t; the library
+ *     carves the workspace and keeps using it until lbm_destroy.  The handle is small host
+ *     memory owned by the library.
+ *   - Array arguments are caller-owned and never retained after the call returns.  For each
+ *     array the `on_device` flag says whether the pointer is a device pointer (used directly by
+ *     kernels on the stream, asynchronous) or a host pointer (copied with cudaMemcpyAsync on the
+ *     stream followed by a stream synchronise before return).
+ *   - Layout: scalar fields are flat with x fastest, index = x + nx*(y + ny*z).  Populations are
+ *     structure-of-arrays [q][N]; vector fields [d][N].
+ *   - Direction order (fixed, part of the ABI):
+ *       D2Q9 : 0 rest; 1..4 = +x,-x,+y,-y; 5..8 = (1,1),(-1,-1),(1,-1),(-1,1)
+ *       D3Q19: 0 rest; 1..6 = +x,-x,+y,-y,+z,-z; 7..10 = (1,1,0),(-1,-1,0),(1,-1,0),(-1,1,0);
+ *              11..14 = (1,0,1),(-1,0,-1),(1,0,-1),(-1,0,1); 15..18 = (0,1,1),(0,-1,-1),(0,1,-1),(0,-1,1)
+ *     lbm_get_lattice returns the tables.
+ *   - Faces: 0 = x-min, 1 = x-max, 2 = y-min, 3 = y-max, 4 = z-min, 5 = z-max.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define LBM_API __attribute__((visibility("default")))
+#else
+#define LBM_API
+#endif
+
+typedef struct lbm lbm_t;
+typedef void* lbm_stream_t; /* a cudaStream_t (NULL = default stream) */
+
+enum lbm_status {
+    LBM_OK = 0,
+    LBM_E_INVALID = -1,     /* bad argument or configuration */
+    LBM_E_UNSUPPORTED = -2, /* valid but not built (e.g. fp64 compute with fp16 storage) */
+    LBM_E_NOMEM = -3,       /* workspace too small or misaligned */
+    LBM_E_CUDA = -4,        /* CUDA runtime error (message in lbm_last_error) */
+    LBM_E_STATE = -5        /* call out of order (e.g. step before init_fields) */
+};
+
+enum lbm_lattice { LBM_D2Q9 = 0, LBM_D3Q19 = 1 };
+
+/* psi(rho), Eq. 12 for the EOS kinds: psi = sqrt(max(0, 2(alpha p_EOS - c_s^2 rho)/g_kk));
+ * LBM_PSI_RHO: psi = rho; LBM_PSI_EXP: psi = exp(-1/rho);
+ * LBM_PSI_SC93: psi = rho0 (1 - exp(-rho/rho0)) (Shan & Chen 1993, cited PAPER.md:121). */
+enum lbm_psi_kind {
+    LBM_PSI_EOS_CS = 0,  /* Carnahan-Starling */
+    LBM_PSI_EOS_PR = 1,  /* Peng-Robinson */
+    LBM_PSI_EOS_VDW = 2, /* van der Waals */
+    LBM_PSI_EOS_RK = 3,  /* Redlich-Kwong */
+    LBM_PSI_EOS_RKS = 4, /* Redlich-Kwong-Soave */
+    LBM_PSI_RHO = 5,
+    LBM_PSI_EXP = 6,
+    LBM_PSI_SC93 = 7
+};
+
+enum lbm_collision { LBM_BGK = 0, LBM_MRT = 1 };      /* Eq. 3 lines 1-2 */
+enum lbm_forcing { LBM_EDM = 0, LBM_SHIFT = 1 };      /* Eq. 5 / velocity shift */
+enum lbm_dtype { LBM_F16 = 0, LBM_F32 = 1, LBM_F64 = 2 };
+enum lbm_face_kind { LBM_FACE_PERIODIC = 0, LBM_FACE_WALL = 1, LBM_FACE_VELOCITY = 2, LBM_FACE_PRESSURE = 3 };
+
+/* flags */
+#define LBM_FLAG_NO_COLLIDE 1u /* f* = f: pure streaming, for the bit-exact permutation test */
+
+typedef struct {
+    int32_t psi_kind; /* lbm_psi_kind */
+    int32_t pad_;
+    double a, b, R, omega; /* EOS parameters (Yuan & Schaefer 2006 as quoted PAPER.md:199, 236) */
+    double T;              /* absolute temperature in lattice units */
+    double alpha;          /* pressure modification parameter alpha^k of Eq. 12 (1 = unmodified) */
+    double rho0;           /* LBM_PSI_SC93 reference density */
+} lbm_eos_t;
+
+typedef struct {
+    double phi, drho; /* Eq. 17: rho_s = phi*rho_ave - drho */
+    double lo, hi;    /* limiter bounds */
+} lbm_wetting_t;
+
+typedef struct {
+    int32_t lattice;      /* lbm_lattice */
+    int32_t nx, ny, nz;   /* nz must be 1 for D2Q9; nx*ny*nz < 2^31 */
+    int32_t n_components; /* 1 or 2 */
+    int32_t periodic[3];  /* per axis; faces of non-periodic axes default to LBM_FACE_WALL */
+    int32_t collision;    /* lbm_collision */
+    int32_t forcing;      /* lbm_forcing */
+    int32_t compute_dtype; /* LBM_F32 or LBM_F64: arithmetic type of every kernel */
+    int32_t store_dtype;   /* LBM_F16 / LBM_F32 / LBM_F64: population storage */
+    uint32_t flags;
+    int32_t pad_;
+    lbm_eos_t eos[2];
+    double G[2][2];          /* g_kk' of Eq. 13; Green's function weights are w_i/c_s^2 (reading R2) */
+    lbm_wetting_t wet[2];
+    double tau[2];           /* BGK relaxation time; with MRT = 1/s_nu (enters the common velocity and LBM_SHIFT) */
+    double mrt_rates[2][19]; /* diagonal of S in the moment order of DESIGN.md R9 (first q entries used) */
+    double rho_ref;          /* populations are stored as f_i - w_i*rho_ref (reading R16); 0 = plain */
+} lbm_config_t;
+
+/* Bytes of device workspace lbm_create needs for cfg; 0 if cfg is invalid. */
+LBM_API size_t lbm_workspace_bytes(const lbm_config_t* cfg);
+
+/* Create a simulation on the current CUDA device.  d_workspace: device pointer, 256-byte aligned,
+ * >= lbm_workspace_bytes(cfg) bytes, owned by the caller, must outlive the handle.  All later device
+ * work is enqueued on `stream`.  Errors: LBM_E_INVALID, LBM_E_UNSUPPORTED, LBM_E_NOMEM, LBM_E_CUDA. */
+LBM_API int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_bytes, lbm_stream_t stream, lbm_t** out);
+
+/* Free the handle.  Never frees the workspace.  NULL is allowed. */
+LBM_API void lbm_destroy(lbm_t* h);
+
+/* Solid mask: N bytes, non-zero = solid (no-slip by halfway bounce-back, reading R13).  Derives the
+ * per-cell link flags and the list of boundary solids (solids with >= 1 fluid neighbour, reading R11).
+ * Must be called before lbm_init_fields (LBM_E_STATE afterwards). */
+LBM_API int lbm_set_solid_mask(lbm_t* h, const uint8_t* mask, int on_device);
+
+/* Boundary condition of one face of a non-periodic axis (reading R10): LBM_FACE_WALL (halfway
+ * bounce-back), LBM_FACE_VELOCITY (bounce-back + 2 w_i rho_w e_i.u_w/c_s^2) or LBM_FACE_PRESSURE
+ * (anti-bounce-back with rho_w; velocity = the boundary node's own).  rho_w[2] per component,
+ * u_w[3].  LBM_E_INVALID for a face of a periodic axis. */
+LBM_API int lbm_set_face_bc(lbm_t* h, int face, int kind, const double* rho_w, const double* u_w);
+
+/* S0: f_i^k = f_eq,i(rho^k, u) at fluid cells (solid cells hold f_eq(1,0) and are never updated);
+ * resets the step counter.  rho[k]: N values each; u: [d][N] or NULL (= 0); dtype: LBM_F32 or LBM_F64
+ * element type of the arrays. */
+LBM_API int lbm_init_fields(lbm_t* h, const void* const* rho, const void* u, int dtype, int on_device);
+
+/* Enqueue n >= 0 time steps (S1..S7) on the stream.  Asynchronous; no host synchronisation. */
+LBM_API int lbm_step(lbm_t* h, int n);
+
+/* S8: rho^k (virtual density at boundary solids, 0 inside solids), u = (sum_k j^k + 1/2 sum_k F^k)/sum_k rho^k
+ * (Eq. 6; 0 at solids), p = c_s^2 sum_k rho^k + 1/2 sum_kk' g_kk' psi^k psi^k' (0 at solids).
+ * Any of rho / u / p may be NULL.  dtype: LBM_F32 or LBM_F64. */
+LBM_API int lbm_get_macroscopic(lbm_t* h, void* const* rho, void* u, void* p, int dtype, int on_device);
+
+/* Parity exports.  Populations are the canonical post-stream f_i(x,t) of component comp, [q][N],
+ * whatever the internal storage is.  dtype LBM_F32 or LBM_F64. */
+LBM_API int lbm_get_populations(lbm_t* h, int comp, void* f, int dtype, int on_device);
+/* Set the post-stream populations directly (tests; doubles as a restart). */
+LBM_API int lbm_set_populations(lbm_t* h, int comp, const void* f, int dtype, int on_device);
+/* Per cell: bit i (1 <= i < q) set <=> the pull of direction i does not read a fluid neighbour
+ * (source solid or beyond a non-periodic face); a solid cell reports exactly 0x80000000. */
+LBM_API int lbm_get_link_flags(lbm_t* h, uint32_t* flags, int on_device);
+/* Boundary-solid list, ascending cell index.  Returns the count (>= 0) or a negative status;
+ * writes min(count, capacity) entries to host memory `out` (may be NULL to query the count). */
+LBM_API int64_t lbm_get_boundary_solids(lbm_t* h, int64_t* out, int64_t capacity);
+/* psi^k field of the current state (compute dtype converted to dtype), N values. */
+LBM_API int lbm_get_psi(lbm_t* h, int comp, void* psi, int dtype, int on_device);
+
+/* Lattice tables: q, e[q][3], w[q], opposite[q].  Host pointers; any may be NULL. */
+LBM_API int lbm_get_lattice(int lattice, int* q, int* e, double* w, int* opposite);
+
+/* sizeof(lbm_config_t) as compiled into the library (ABI check for bindings). */
+LBM_API size_t lbm_config_bytes(void);
+
+/* Bookkeeping. */
+LBM_API int64_t lbm_steps_done(const lbm_t* h);
+LBM_API int64_t lbm_kernel_launches(const lbm_t* h); /* kernels launched by this handle so far */
+LBM_API const char* lbm_last_error(const lbm_t* h);
+LBM_API const char* lbm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_B200_H */

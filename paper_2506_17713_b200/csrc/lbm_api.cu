@@ -1,0 +1,729 @@
+// lbm_api.cu -- the C-ABI of include/lbm.h: configuration checks, workspace carving, boundary
+// preprocessing kernels, and the launch sequence of the hot loop (K1 -> K1b -> K2 per step).
+// No device memory is allocated here; everything lives in the caller's workspace.
+#include "../../include/lbm.h"
+#include "lbm_launch.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace lbmk;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+constexpr int CHUNK_CELLS = 1 << 21;  // staging granularity for host / converted transfers
+
+size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+size_t dtype_bytes(int dt) { return dt == LBM_F16 ? 2 : dt == LBM_F32 ? 4 : 8; }
+
+struct Carve {
+    size_t f[2], psi, rho, flags, bsolid, mask, counter, stage_a, stage_b, total;
+};
+
+}  // namespace
+
+struct lbm {
+    lbm_config_t cfg;
+    int q, d, N;
+    long long plane;
+    size_t sbytes, cbytes;
+    cudaStream_t stream;
+    char* ws;
+    Carve cv;
+    int cur;
+    int local;
+    bool initialized, has_solid, bnd, dirty, force_rho;
+    int nbsolid;
+    int face_kind[6];
+    double face_rho[6][2], face_u[6][3];
+    int64_t steps, launches;
+    std::string err;
+};
+
+namespace {
+
+int q_of(int lattice) { return lattice == LBM_D2Q9 ? 9 : 19; }
+
+int check_config(const lbm_config_t* c) {
+    if (!c) return LBM_E_INVALID;
+    if (c->lattice != LBM_D2Q9 && c->lattice != LBM_D3Q19) return LBM_E_INVALID;
+    if (c->nx < 1 || c->ny < 1 || c->nz < 1) return LBM_E_INVALID;
+    if (c->lattice == LBM_D2Q9 && c->nz != 1) return LBM_E_INVALID;
+    if ((long long)c->nx * c->ny * c->nz >= (1LL << 31) - 64) return LBM_E_INVALID;
+    if (c->n_components < 1 || c->n_components > 2) return LBM_E_INVALID;
+    if (c->collision != LBM_BGK && c->collision != LBM_MRT) return LBM_E_INVALID;
+    if (c->forcing != LBM_EDM && c->forcing != LBM_SHIFT) return LBM_E_INVALID;
+    if (c->compute_dtype != LBM_F32 && c->compute_dtype != LBM_F64) return LBM_E_INVALID;
+    if (c->store_dtype != LBM_F16 && c->store_dtype != LBM_F32 && c->store_dtype != LBM_F64) return LBM_E_INVALID;
+    if (c->compute_dtype == LBM_F32 && c->store_dtype == LBM_F64) return LBM_E_INVALID;
+    if (c->compute_dtype == LBM_F64 && c->store_dtype == LBM_F16) return LBM_E_UNSUPPORTED;
+    for (int k = 0; k < c->n_components; ++k) {
+        const lbm_eos_t& e = c->eos[k];
+        if (e.psi_kind < LBM_PSI_EOS_CS || e.psi_kind > LBM_PSI_SC93) return LBM_E_INVALID;
+        if (e.psi_kind <= LBM_PSI_EOS_RKS) {
+            if (!(c->G[k][k] < 0.0)) return LBM_E_INVALID;  // R4: g_kk < 0 under the root
+            if (!(e.b > 0.0) || !(e.R > 0.0) || !(e.T > 0.0)) return LBM_E_INVALID;
+        }
+        if (e.psi_kind == LBM_PSI_SC93 && !(e.rho0 > 0.0)) return LBM_E_INVALID;
+        if (!(c->tau[k] > 0.5)) return LBM_E_INVALID;
+    }
+    return LBM_OK;
+}
+
+Carve carve(const lbm_config_t& c) {
+    Carve v{};
+    const size_t N = (size_t)c.nx * c.ny * c.nz;
+    const size_t q = q_of(c.lattice), nc = c.n_components;
+    const size_t plane = (N + 63) / 64 * 64;
+    const size_t sb = dtype_bytes(c.store_dtype), cb = dtype_bytes(c.compute_dtype);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+    v.f[0] = take(nc * q * plane * sb);
+    v.f[1] = take(nc * q * plane * sb);
+    v.psi = take(nc * N * cb);
+    v.rho = take(nc * N * cb);
+    v.flags = take(N * 4);
+    v.bsolid = take(N * 4);
+    v.mask = take(N);
+    v.counter = take(256);
+    const size_t chunk = std::min<size_t>(N, CHUNK_CELLS);
+    v.stage_a = take(q * chunk * 8);
+    v.stage_b = take(q * chunk * 8);
+    v.total = off;
+    return v;
+}
+
+double eos_tc(int kind, double a, double b, double R) {
+    switch (kind) {
+        case LBM_PSI_EOS_CS: return 0.3773 * a / (b * R);
+        case LBM_PSI_EOS_PR: return 0.0778 / 0.45724 * a / (b * R);
+        case LBM_PSI_EOS_VDW: return 8.0 / 27.0 * a / (b * R);
+        case LBM_PSI_EOS_RK: return std::cbrt(std::pow(0.08664 / 0.42748 * a / (b * R), 2.0));
+        case LBM_PSI_EOS_RKS: return 0.08664 / 0.42748 * a / (b * R);
+    }
+    return 1.0;
+}
+
+template <class L>
+void lattice_weights(double* w) {
+    for (int i = 0; i < L::Q; ++i) w[i] = (double)L::WN[i] / (double)L::WD;
+}
+
+template <class CT>
+KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
+    KParams<CT> p;
+    std::memset(&p, 0, sizeof p);
+    const lbm_config_t& c = h->cfg;
+    p.nx = c.nx; p.ny = c.ny; p.nz = c.nz; p.N = h->N;
+    for (int a = 0; a < 3; ++a) p.periodic[a] = c.periodic[a] ? 1 : 0;
+    p.plane = h->plane;
+    p.f_in = h->ws + h->cv.f[in_buf];
+    p.f_out = h->ws + h->cv.f[out_buf];
+    p.psi = reinterpret_cast<CT*>(h->ws + h->cv.psi);
+    p.rho = reinterpret_cast<CT*>(h->ws + h->cv.rho);
+    p.flags = reinterpret_cast<const uint32_t*>(h->ws + h->cv.flags);
+    p.bsolid = reinterpret_cast<const int*>(h->ws + h->cv.bsolid);
+    p.nbsolid = h->nbsolid;
+    p.local = h->local;
+    p.no_collide = (c.flags & LBM_FLAG_NO_COLLIDE) ? 1 : 0;
+    p.forcing = c.forcing == LBM_SHIFT ? 1 : 0;
+    p.write_rho = (h->nbsolid > 0 || h->force_rho) ? 1 : 0;
+    double w[19];
+    if (c.lattice == LBM_D2Q9) lattice_weights<D2Q9>(w);
+    else lattice_weights<D3Q19>(w);
+    for (int i = 0; i < h->q; ++i) p.wref[i] = (CT)(w[i] * c.rho_ref);
+    for (int k = 0; k < c.n_components; ++k) {
+        p.tau[k] = (CT)c.tau[k];
+        p.inv_tau[k] = (CT)(1.0 / c.tau[k]);
+        for (int kp = 0; kp < c.n_components; ++kp) p.G[k][kp] = (CT)c.G[k][kp];
+        for (int r = 0; r < h->q; ++r) p.mrt_s[k][r] = (CT)c.mrt_rates[k][r];
+        const lbm_eos_t& e = c.eos[k];
+        p.psi_kind[k] = e.psi_kind;
+        p.eos_a[k] = (CT)e.a;
+        p.eos_b[k] = (CT)e.b;
+        p.eos_RT[k] = (CT)(e.R * e.T);
+        p.eos_sqrtT[k] = (CT)std::sqrt(e.T > 0 ? e.T : 1.0);
+        p.eos_alpha[k] = (CT)e.alpha;
+        p.eos_rho0[k] = (CT)e.rho0;
+        p.eos_inv_gkk2[k] = c.G[k][k] != 0.0 ? (CT)(2.0 / c.G[k][k]) : (CT)0;
+        double aalpha = e.a;
+        if (e.psi_kind == LBM_PSI_EOS_PR || e.psi_kind == LBM_PSI_EOS_RKS) {
+            const double tc = eos_tc(e.psi_kind, e.a, e.b, e.R);
+            const double m = e.psi_kind == LBM_PSI_EOS_PR
+                                 ? 0.37464 + 1.54226 * e.omega - 0.26992 * e.omega * e.omega
+                                 : 0.480 + 1.574 * e.omega - 0.176 * e.omega * e.omega;
+            const double s = 1.0 + m * (1.0 - std::sqrt(e.T / tc));
+            aalpha = e.a * s * s;
+        }
+        p.eos_aalpha[k] = (CT)aalpha;
+        p.wet_phi[k] = (CT)c.wet[k].phi;
+        p.wet_drho[k] = (CT)c.wet[k].drho;
+        p.wet_lo[k] = (CT)c.wet[k].lo;
+        p.wet_hi[k] = (CT)c.wet[k].hi;
+    }
+    for (int fc = 0; fc < 6; ++fc) {
+        p.face_kind[fc] = h->face_kind[fc];
+        for (int k = 0; k < 2; ++k) p.face_rho[fc][k] = (CT)h->face_rho[fc][k];
+        for (int a = 0; a < 3; ++a) p.face_u[fc][a] = (CT)h->face_u[fc][a];
+    }
+    return p;
+}
+
+// ---------------------------------------------------------------- boundary preprocessing kernels
+struct Geo {
+    int nx, ny, nz, N;
+    int periodic[3];
+    int face_kind[6];
+};
+
+// link flags (integer-only): bit i = pull of direction i has no fluid source; SOLID_BIT; FACEBC_BIT
+template <class L>
+__global__ void k_build_flags(Geo g, const uint8_t* __restrict__ mask, uint32_t* __restrict__ flags) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= g.N) return;
+    if (mask && mask[id]) { flags[id] = SOLID_BIT; return; }
+    const int x = id % g.nx, t = id / g.nx, y = t % g.ny, z = t / g.ny;
+    const int n[3] = {g.nx, g.ny, g.nz};
+    uint32_t fl = 0;
+    static_for<1, L::Q>([&](auto I) {
+        constexpr int i = I;
+        int pc[3] = {x - L::E[i][0], y - L::E[i][1], z - L::E[i][2]};
+        int face = -1;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (pc[a] < 0) {
+                if (g.periodic[a]) pc[a] += n[a];
+                else { if (face < 0) face = 2 * a; pc[a] = 0; }
+            } else if (pc[a] >= n[a]) {
+                if (g.periodic[a]) pc[a] -= n[a];
+                else { if (face < 0) face = 2 * a + 1; pc[a] = n[a] - 1; }
+            }
+        }
+        if (face >= 0) {
+            fl |= 1u << i;
+            if (g.face_kind[face] == FACE_VELOCITY || g.face_kind[face] == FACE_PRESSURE) fl |= FACEBC_BIT;
+        } else if (mask && mask[pc[0] + g.nx * (pc[1] + g.ny * pc[2])]) {
+            fl |= 1u << i;
+        }
+    });
+    flags[id] = fl;
+}
+
+// boundary solids: solid cells with >= 1 fluid neighbour under wrap/clamp indexing (R11)
+template <class L>
+__global__ void k_list_boundary_solids(Geo g, const uint32_t* __restrict__ flags, int* __restrict__ list, int* counter) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= g.N) return;
+    if (!(flags[id] & SOLID_BIT)) return;
+    const int x = id % g.nx, t = id / g.nx, y = t % g.ny, z = t / g.ny;
+    const int n[3] = {g.nx, g.ny, g.nz};
+    bool any = false;
+    static_for<1, L::Q>([&](auto I) {
+        constexpr int i = I;
+        int pc[3] = {x + L::E[i][0], y + L::E[i][1], z + L::E[i][2]};
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (pc[a] < 0) pc[a] = g.periodic[a] ? pc[a] + n[a] : 0;
+            if (pc[a] >= n[a]) pc[a] = g.periodic[a] ? pc[a] - n[a] : n[a] - 1;
+        }
+        if (!(flags[pc[0] + g.nx * (pc[1] + g.ny * pc[2])] & SOLID_BIT)) any = true;
+    });
+    if (any) list[atomicAdd(counter, 1)] = id;
+}
+
+__global__ void k_export_flags(int N, const uint32_t* __restrict__ in, uint32_t* __restrict__ out) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id < N) out[id] = in[id] & (SOLID_BIT | LINK_MASK);
+}
+
+template <class TI, class TO>
+__global__ void k_convert(const TI* __restrict__ in, TO* __restrict__ out, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (TO)in[i];
+}
+
+// ---------------------------------------------------------------- helpers
+int fail(lbm* h, int code, const char* what) {
+    h->err = what;
+    return code;
+}
+int cuda_fail(lbm* h, cudaError_t e, const char* where) {
+    h->err = std::string(where) + ": " + cudaGetErrorString(e);
+    return LBM_E_CUDA;
+}
+#define CU(call)                                                  \
+    do {                                                          \
+        cudaError_t e_ = (call);                                  \
+        if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);    \
+    } while (0)
+
+typedef cudaError_t (*launch_fn)(const LaunchArgs&);
+
+launch_fn pick_launch(const lbm_config_t& c) {
+    const bool d2 = c.lattice == LBM_D2Q9;
+    if (c.compute_dtype == LBM_F32) {
+        if (c.store_dtype == LBM_F32) return d2 ? &launch<D2Q9, float, float> : &launch<D3Q19, float, float>;
+        if (c.store_dtype == LBM_F16) return d2 ? &launch<D2Q9, float, __half> : &launch<D3Q19, float, __half>;
+    } else {
+        if (c.store_dtype == LBM_F64) return d2 ? &launch<D2Q9, double, double> : &launch<D3Q19, double, double>;
+        if (c.store_dtype == LBM_F32) return d2 ? &launch<D2Q9, double, float> : &launch<D3Q19, double, float>;
+    }
+    return nullptr;
+}
+
+// in_buf / out_buf: which population buffer the kernel reads / writes (-1 = current / the other one)
+int do_launch(lbm* h, int op, const void* a0 = nullptr, const void* a1 = nullptr, void* a2 = nullptr, int i0 = 0,
+              int in_buf = -1, int out_buf = -1) {
+    if (in_buf < 0) in_buf = h->cur;
+    if (out_buf < 0) out_buf = h->cur ^ 1;
+    LaunchArgs a;
+    a.op = op;
+    a.nc = h->cfg.n_components;
+    a.coll = h->cfg.collision == LBM_MRT ? 1 : 0;
+    a.bnd = h->bnd ? 1 : 0;
+    a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
+    a.stream = h->stream;
+    launch_fn fn = pick_launch(h->cfg);
+    if (!fn) return fail(h, LBM_E_UNSUPPORTED, "dtype combination not built");
+    cudaError_t e;
+    if (h->cfg.compute_dtype == LBM_F32) {
+        KParams<float> p = make_params<float>(h, in_buf, out_buf);
+        a.params = &p;
+        e = fn(a);
+    } else {
+        KParams<double> p = make_params<double>(h, in_buf, out_buf);
+        a.params = &p;
+        e = fn(a);
+    }
+    if (e != cudaSuccess) return cuda_fail(h, e, "kernel launch");
+    if (!(op == OP_VIRTUAL && h->nbsolid == 0)) h->launches++;
+    return LBM_OK;
+}
+
+// FieldIO<CT> is the same layout for float and double (pointers + ints): fill it through void*
+struct FieldIOAny {
+    const void* in[19];
+    void* out;
+    long long out_stride;
+    int c0, cnt;
+};
+static_assert(sizeof(FieldIOAny) == sizeof(FieldIO<float>) && sizeof(FieldIOAny) == sizeof(FieldIO<double>),
+              "FieldIO layout");
+
+Geo make_geo(const lbm* h) {
+    Geo g;
+    g.nx = h->cfg.nx; g.ny = h->cfg.ny; g.nz = h->cfg.nz; g.N = h->N;
+    for (int a = 0; a < 3; ++a) g.periodic[a] = h->cfg.periodic[a] ? 1 : 0;
+    for (int f = 0; f < 6; ++f) g.face_kind[f] = h->face_kind[f];
+    return g;
+}
+
+// (re)build link flags and the boundary-solid list after a mask / face change
+int prepare(lbm* h) {
+    if (!h->dirty) return LBM_OK;
+    h->bnd = h->has_solid || !h->cfg.periodic[0] || !h->cfg.periodic[1] || (h->d == 3 && !h->cfg.periodic[2]);
+    h->nbsolid = 0;
+    CU(cudaMemsetAsync(h->ws + h->cv.psi, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
+    CU(cudaMemsetAsync(h->ws + h->cv.rho, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
+    if (h->bnd) {
+        const Geo g = make_geo(h);
+        const uint8_t* mask = h->has_solid ? reinterpret_cast<const uint8_t*>(h->ws + h->cv.mask) : nullptr;
+        uint32_t* flags = reinterpret_cast<uint32_t*>(h->ws + h->cv.flags);
+        int* list = reinterpret_cast<int*>(h->ws + h->cv.bsolid);
+        int* counter = reinterpret_cast<int*>(h->ws + h->cv.counter);
+        const int block = 256, grid = (h->N + block - 1) / block;
+        CU(cudaMemsetAsync(counter, 0, sizeof(int), h->stream));
+        if (h->d == 2) k_build_flags<D2Q9><<<grid, block, 0, h->stream>>>(g, mask, flags);
+        else k_build_flags<D3Q19><<<grid, block, 0, h->stream>>>(g, mask, flags);
+        CU(cudaGetLastError());
+        h->launches++;
+        if (h->has_solid) {
+            if (h->d == 2) k_list_boundary_solids<D2Q9><<<grid, block, 0, h->stream>>>(g, flags, list, counter);
+            else k_list_boundary_solids<D3Q19><<<grid, block, 0, h->stream>>>(g, flags, list, counter);
+            CU(cudaGetLastError());
+            h->launches++;
+            int cnt = 0;
+            CU(cudaMemcpyAsync(&cnt, counter, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+            CU(cudaStreamSynchronize(h->stream));
+            h->nbsolid = cnt;
+        }
+    }
+    h->dirty = false;
+    return LBM_OK;
+}
+
+template <class TI, class TO>
+int convert(lbm* h, const void* in, void* out, long long n) {
+    const int block = 256;
+    k_convert<TI, TO><<<(unsigned)((n + block - 1) / block), block, 0, h->stream>>>(static_cast<const TI*>(in),
+                                                                                  static_cast<TO*>(out), n);
+    CU(cudaGetLastError());
+    h->launches++;
+    return LBM_OK;
+}
+
+// Bring `n` values of element type `dtype` (host or device) into the compute dtype on the device.
+// Returns a device pointer in *out: the source itself when no copy/convert is needed, else stage_a/stage_b.
+int fetch_input(lbm* h, const void* src, long long n, int dtype, int on_device, char* stage_raw, char* stage_ct,
+                const void** out) {
+    const size_t eb = dtype_bytes(dtype);
+    const void* dev = src;
+    if (!on_device) {
+        CU(cudaMemcpyAsync(stage_raw, src, (size_t)n * eb, cudaMemcpyHostToDevice, h->stream));
+        dev = stage_raw;
+    }
+    if (dtype == h->cfg.compute_dtype) { *out = dev; return LBM_OK; }
+    int rc = dtype == LBM_F32 ? convert<float, double>(h, dev, stage_ct, n) : convert<double, float>(h, dev, stage_ct, n);
+    if (rc) return rc;
+    *out = stage_ct;
+    return LBM_OK;
+}
+
+// Deliver `n` compute-dtype values at device pointer `dev` to dst (host or device) as `dtype`.
+int deliver_output(lbm* h, const void* dev, long long n, int dtype, int on_device, char* stage_conv, void* dst) {
+    const void* src = dev;
+    if (dtype != h->cfg.compute_dtype) {
+        void* conv = on_device ? dst : stage_conv;
+        int rc = dtype == LBM_F32 ? convert<double, float>(h, dev, conv, n) : convert<float, double>(h, dev, conv, n);
+        if (rc) return rc;
+        if (on_device) return LBM_OK;
+        src = conv;
+    }
+    if (src != dst)
+        CU(cudaMemcpyAsync(dst, src, (size_t)n * dtype_bytes(dtype),
+                           on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+    return LBM_OK;
+}
+
+}  // namespace
+
+// ==================================================================== C ABI
+extern "C" {
+
+size_t lbm_workspace_bytes(const lbm_config_t* cfg) {
+    if (check_config(cfg) != LBM_OK) return 0;
+    return carve(*cfg).total;
+}
+
+int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_bytes, lbm_stream_t stream, lbm_t** out) {
+    if (!out) return LBM_E_INVALID;
+    *out = nullptr;
+    int rc = check_config(cfg);
+    if (rc != LBM_OK) return rc;
+    if (!pick_launch(*cfg)) return LBM_E_UNSUPPORTED;
+    const Carve cv = carve(*cfg);
+    if (!d_workspace || workspace_bytes < cv.total || (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) != 0)
+        return LBM_E_NOMEM;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LBM_E_CUDA;  // no CPU fallback
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, d_workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return LBM_E_INVALID;
+    }
+    lbm* h = new (std::nothrow) lbm();
+    if (!h) return LBM_E_NOMEM;
+    h->cfg = *cfg;
+    h->q = q_of(cfg->lattice);
+    h->d = cfg->lattice == LBM_D2Q9 ? 2 : 3;
+    h->N = cfg->nx * cfg->ny * cfg->nz;
+    h->plane = ((long long)h->N + 63) / 64 * 64;
+    h->sbytes = dtype_bytes(cfg->store_dtype);
+    h->cbytes = dtype_bytes(cfg->compute_dtype);
+    h->stream = static_cast<cudaStream_t>(stream);
+    h->ws = static_cast<char*>(d_workspace);
+    h->cv = cv;
+    h->cur = 0;
+    h->local = 1;
+    h->initialized = false;
+    h->has_solid = false;
+    h->dirty = true;
+    h->bnd = false;
+    h->force_rho = false;
+    h->nbsolid = 0;
+    h->steps = 0;
+    h->launches = 0;
+    for (int f = 0; f < 6; ++f) {
+        h->face_kind[f] = cfg->periodic[f / 2] ? LBM_FACE_PERIODIC : LBM_FACE_WALL;
+        h->face_rho[f][0] = h->face_rho[f][1] = 1.0;
+        h->face_u[f][0] = h->face_u[f][1] = h->face_u[f][2] = 0.0;
+    }
+    *out = h;
+    return LBM_OK;
+}
+
+void lbm_destroy(lbm_t* h) { delete h; }
+
+int lbm_set_solid_mask(lbm_t* h, const uint8_t* mask, int on_device) {
+    if (!h || !mask) return LBM_E_INVALID;
+    if (h->initialized) return fail(h, LBM_E_STATE, "lbm_set_solid_mask must precede lbm_init_fields");
+    CU(cudaMemcpyAsync(h->ws + h->cv.mask, mask, (size_t)h->N,
+                       on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+    if (!on_device) CU(cudaStreamSynchronize(h->stream));
+    h->has_solid = true;
+    h->dirty = true;
+    return LBM_OK;
+}
+
+int lbm_set_face_bc(lbm_t* h, int face, int kind, const double* rho_w, const double* u_w) {
+    if (!h) return LBM_E_INVALID;
+    if (face < 0 || face >= 2 * h->d) return fail(h, LBM_E_INVALID, "face out of range");
+    if (h->cfg.periodic[face / 2]) return fail(h, LBM_E_INVALID, "face belongs to a periodic axis");
+    if (kind != LBM_FACE_WALL && kind != LBM_FACE_VELOCITY && kind != LBM_FACE_PRESSURE)
+        return fail(h, LBM_E_INVALID, "face kind");
+    h->face_kind[face] = kind;
+    for (int k = 0; k < 2; ++k) h->face_rho[face][k] = rho_w ? rho_w[k] : 1.0;
+    for (int a = 0; a < 3; ++a) h->face_u[face][a] = u_w ? u_w[a] : 0.0;
+    h->dirty = true;
+    return LBM_OK;
+}
+
+int lbm_init_fields(lbm_t* h, const void* const* rho, const void* u, int dtype, int on_device) {
+    if (!h || !rho) return LBM_E_INVALID;
+    if (dtype != LBM_F32 && dtype != LBM_F64) return fail(h, LBM_E_INVALID, "dtype");
+    int rc = prepare(h);
+    if (rc) return rc;
+    const int nc = h->cfg.n_components;
+    for (int k = 0; k < nc; ++k)
+        if (!rho[k]) return fail(h, LBM_E_INVALID, "rho[k] is NULL");
+    const size_t eb = dtype_bytes(dtype);
+    const int chunk = std::min(h->N, CHUNK_CELLS);
+    for (int c0 = 0; c0 < h->N; c0 += chunk) {
+        const int cnt = std::min(chunk, h->N - c0);
+        FieldIOAny io;
+        std::memset(&io, 0, sizeof io);
+        io.c0 = c0;
+        io.cnt = cnt;
+        // slot s of the staging areas: raw bytes in stage_a, compute-dtype values in stage_b
+        auto stage = [&](int slot, const void* src, const void** dev) {
+            return fetch_input(h, src, cnt, dtype, on_device, h->ws + h->cv.stage_a + (size_t)slot * chunk * 8,
+                               h->ws + h->cv.stage_b + (size_t)slot * chunk * 8, dev);
+        };
+        for (int k = 0; k < nc; ++k)
+            if ((rc = stage(k, static_cast<const char*>(rho[k]) + (size_t)c0 * eb, &io.in[k]))) return rc;
+        if (u)
+            for (int a = 0; a < h->d; ++a)
+                if ((rc = stage(2 + a, static_cast<const char*>(u) + ((size_t)a * h->N + c0) * eb, &io.in[2 + a])))
+                    return rc;
+        // fill the CURRENT buffer; solid cells are written to the other buffer too
+        rc = do_launch(h, OP_INIT, &io, nullptr, h->ws + h->cv.f[h->cur ^ 1], h->bnd ? 1 : 0, h->cur ^ 1, h->cur);
+        if (rc) return rc;
+        if (!on_device) CU(cudaStreamSynchronize(h->stream));  // staging slots are reused by the next chunk
+    }
+    h->local = 1;
+    h->steps = 0;
+    h->initialized = true;
+    return LBM_OK;
+}
+
+int lbm_step(lbm_t* h, int n) {
+    if (!h || n < 0) return LBM_E_INVALID;
+    if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_step before lbm_init_fields");
+    int rc = prepare(h);
+    if (rc) return rc;
+    for (int s = 0; s < n; ++s) {
+        if (!(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) {
+            if ((rc = do_launch(h, OP_MOMENTS))) return rc;
+            if (h->nbsolid > 0 && (rc = do_launch(h, OP_VIRTUAL))) return rc;
+        }
+        if ((rc = do_launch(h, OP_STEP))) return rc;
+        h->cur ^= 1;
+        h->local = 0;
+        h->steps++;
+    }
+    return LBM_OK;
+}
+
+int lbm_get_macroscopic(lbm_t* h, void* const* rho, void* u, void* p, int dtype, int on_device) {
+    if (!h) return LBM_E_INVALID;
+    if (dtype != LBM_F32 && dtype != LBM_F64) return fail(h, LBM_E_INVALID, "dtype");
+    if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_get_macroscopic before lbm_init_fields");
+    int rc = prepare(h);
+    if (rc) return rc;
+    const int nc = h->cfg.n_components;
+    // refresh rho / psi of the current state: K1 (with rho output) and K1b
+    h->force_rho = true;
+    rc = do_launch(h, OP_MOMENTS);
+    h->force_rho = false;
+    if (rc) return rc;
+    if (h->nbsolid > 0 && (rc = do_launch(h, OP_VIRTUAL))) return rc;
+    // u and p go to the free population buffer ((d+1) compute-dtype fields always fit in q planes)
+    char* scratch = h->ws + h->cv.f[h->cur ^ 1];
+    char* u_dev = scratch;
+    char* p_dev = scratch + (size_t)h->d * h->N * h->cbytes;
+    if (u || p) {
+        rc = do_launch(h, OP_EXPORT_MACRO, u ? u_dev : nullptr, p ? p_dev : nullptr);
+        if (rc) return rc;
+    }
+    const size_t eb = dtype_bytes(dtype);
+    const int chunk = std::min(h->N, CHUNK_CELLS);
+    auto deliver_field = [&](const char* dev, void* dst) -> int {
+        for (int c0 = 0; c0 < h->N; c0 += chunk) {
+            const int cnt = std::min(chunk, h->N - c0);
+            int r = deliver_output(h, dev + (size_t)c0 * h->cbytes, cnt, dtype, on_device, h->ws + h->cv.stage_a,
+                                   static_cast<char*>(dst) + (size_t)c0 * eb);
+            if (r) return r;
+            if (!on_device && dtype != h->cfg.compute_dtype) CU(cudaStreamSynchronize(h->stream));
+        }
+        return LBM_OK;
+    };
+    if (rho)
+        for (int k = 0; k < nc; ++k)
+            if (rho[k] && (rc = deliver_field(h->ws + h->cv.rho + (size_t)k * h->N * h->cbytes, rho[k]))) return rc;
+    if (u)
+        for (int a = 0; a < h->d; ++a)
+            if ((rc = deliver_field(u_dev + (size_t)a * h->N * h->cbytes, static_cast<char*>(u) + (size_t)a * h->N * eb)))
+                return rc;
+    if (p && (rc = deliver_field(p_dev, p))) return rc;
+    if (!on_device) CU(cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+int lbm_get_populations(lbm_t* h, int comp, void* f, int dtype, int on_device) {
+    if (!h || !f) return LBM_E_INVALID;
+    if (comp < 0 || comp >= h->cfg.n_components) return fail(h, LBM_E_INVALID, "component");
+    if (dtype != LBM_F32 && dtype != LBM_F64) return fail(h, LBM_E_INVALID, "dtype");
+    if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_get_populations before lbm_init_fields");
+    int rc = prepare(h);
+    if (rc) return rc;
+    const size_t eb = dtype_bytes(dtype);
+    if (on_device && dtype == h->cfg.compute_dtype) {  // straight into the caller's array
+        FieldIOAny io;
+        std::memset(&io, 0, sizeof io);
+        io.out = f; io.out_stride = h->N; io.c0 = 0; io.cnt = h->N;
+        return do_launch(h, OP_EXPORT_POP, &io, nullptr, nullptr, comp);
+    }
+    const int chunk = std::min(h->N, CHUNK_CELLS);
+    for (int c0 = 0; c0 < h->N; c0 += chunk) {
+        const int cnt = std::min(chunk, h->N - c0);
+        FieldIOAny io;
+        std::memset(&io, 0, sizeof io);
+        io.out = h->ws + h->cv.stage_b; io.out_stride = cnt; io.c0 = c0; io.cnt = cnt;
+        if ((rc = do_launch(h, OP_EXPORT_POP, &io, nullptr, nullptr, comp))) return rc;
+        for (int i = 0; i < h->q; ++i) {
+            rc = deliver_output(h, h->ws + h->cv.stage_b + (size_t)i * cnt * h->cbytes, cnt, dtype, on_device,
+                                h->ws + h->cv.stage_a + (size_t)i * chunk * 8,
+                                static_cast<char*>(f) + ((size_t)i * h->N + c0) * eb);
+            if (rc) return rc;
+        }
+        if (!on_device) CU(cudaStreamSynchronize(h->stream));
+    }
+    return LBM_OK;
+}
+
+int lbm_set_populations(lbm_t* h, int comp, const void* f, int dtype, int on_device) {
+    if (!h || !f) return LBM_E_INVALID;
+    if (comp < 0 || comp >= h->cfg.n_components) return fail(h, LBM_E_INVALID, "component");
+    if (dtype != LBM_F32 && dtype != LBM_F64) return fail(h, LBM_E_INVALID, "dtype");
+    if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_set_populations before lbm_init_fields");
+    if (!h->local) return fail(h, LBM_E_STATE, "lbm_set_populations is only valid right after lbm_init_fields");
+    int rc = prepare(h);
+    if (rc) return rc;
+    const size_t eb = dtype_bytes(dtype);
+    const int chunk = std::min(h->N, CHUNK_CELLS);
+    for (int c0 = 0; c0 < h->N; c0 += chunk) {
+        const int cnt = std::min(chunk, h->N - c0);
+        FieldIOAny io;
+        std::memset(&io, 0, sizeof io);
+        io.c0 = c0; io.cnt = cnt;
+        for (int i = 0; i < h->q; ++i) {
+            rc = fetch_input(h, static_cast<const char*>(f) + ((size_t)i * h->N + c0) * eb, cnt, dtype, on_device,
+                             h->ws + h->cv.stage_a + (size_t)i * chunk * 8, h->ws + h->cv.stage_b + (size_t)i * chunk * 8,
+                             &io.in[i]);
+            if (rc) return rc;
+        }
+        rc = do_launch(h, OP_IMPORT_POP, &io, nullptr, h->ws + h->cv.f[h->cur ^ 1], comp, h->cur ^ 1, h->cur);
+        if (rc) return rc;
+        if (!on_device) CU(cudaStreamSynchronize(h->stream));
+    }
+    return LBM_OK;
+}
+
+int lbm_get_link_flags(lbm_t* h, uint32_t* flags, int on_device) {
+    if (!h || !flags) return LBM_E_INVALID;
+    int rc = prepare(h);
+    if (rc) return rc;
+    uint32_t* tmp = reinterpret_cast<uint32_t*>(h->ws + h->cv.f[h->cur ^ 1]);
+    if (!h->bnd) {
+        CU(cudaMemsetAsync(on_device ? (void*)flags : (void*)tmp, 0, (size_t)h->N * 4, h->stream));
+    } else {
+        const int block = 256;
+        k_export_flags<<<(h->N + block - 1) / block, block, 0, h->stream>>>(
+            h->N, reinterpret_cast<const uint32_t*>(h->ws + h->cv.flags), on_device ? flags : tmp);
+        CU(cudaGetLastError());
+        h->launches++;
+    }
+    if (!on_device) {
+        CU(cudaMemcpyAsync(flags, tmp, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    return LBM_OK;
+}
+
+int64_t lbm_get_boundary_solids(lbm_t* h, int64_t* out, int64_t capacity) {
+    if (!h) return LBM_E_INVALID;
+    int rc = prepare(h);
+    if (rc) return rc;
+    if (!out || h->nbsolid == 0) return h->nbsolid;
+    std::vector<int> tmp((size_t)h->nbsolid);
+    cudaError_t e = cudaMemcpyAsync(tmp.data(), h->ws + h->cv.bsolid, (size_t)h->nbsolid * 4, cudaMemcpyDeviceToHost,
+                                    h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "boundary solid readback");
+    std::sort(tmp.begin(), tmp.end());
+    for (int64_t b = 0; b < h->nbsolid && b < capacity; ++b) out[b] = tmp[(size_t)b];
+    return h->nbsolid;
+}
+
+int lbm_get_psi(lbm_t* h, int comp, void* psi, int dtype, int on_device) {
+    if (!h || !psi) return LBM_E_INVALID;
+    if (comp < 0 || comp >= h->cfg.n_components) return fail(h, LBM_E_INVALID, "component");
+    if (dtype != LBM_F32 && dtype != LBM_F64) return fail(h, LBM_E_INVALID, "dtype");
+    if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_get_psi before lbm_init_fields");
+    int rc = prepare(h);
+    if (rc) return rc;
+    if ((rc = do_launch(h, OP_MOMENTS))) return rc;
+    if (h->nbsolid > 0 && (rc = do_launch(h, OP_VIRTUAL))) return rc;
+    const size_t eb = dtype_bytes(dtype);
+    const int chunk = std::min(h->N, CHUNK_CELLS);
+    const char* dev = h->ws + h->cv.psi + (size_t)comp * h->N * h->cbytes;
+    for (int c0 = 0; c0 < h->N; c0 += chunk) {
+        const int cnt = std::min(chunk, h->N - c0);
+        rc = deliver_output(h, dev + (size_t)c0 * h->cbytes, cnt, dtype, on_device, h->ws + h->cv.stage_a,
+                            static_cast<char*>(psi) + (size_t)c0 * eb);
+        if (rc) return rc;
+        if (!on_device && dtype != h->cfg.compute_dtype) CU(cudaStreamSynchronize(h->stream));
+    }
+    if (!on_device) CU(cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+int lbm_get_lattice(int lattice, int* q, int* e, double* w, int* opposite_out) {
+    if (lattice != LBM_D2Q9 && lattice != LBM_D3Q19) return LBM_E_INVALID;
+    auto fill = [&](auto L) {
+        using LT = decltype(L);
+        if (q) *q = LT::Q;
+        for (int i = 0; i < LT::Q; ++i) {
+            if (e) for (int a = 0; a < 3; ++a) e[3 * i + a] = LT::E[i][a];
+            if (w) w[i] = (double)LT::WN[i] / (double)LT::WD;
+            if (opposite_out) opposite_out[i] = opposite<LT>(i);
+        }
+    };
+    if (lattice == LBM_D2Q9) fill(D2Q9{});
+    else fill(D3Q19{});
+    return LBM_OK;
+}
+
+int64_t lbm_steps_done(const lbm_t* h) { return h ? h->steps : LBM_E_INVALID; }
+int64_t lbm_kernel_launches(const lbm_t* h) { return h ? h->launches : LBM_E_INVALID; }
+const char* lbm_last_error(const lbm_t* h) { return h ? h->err.c_str() : "null handle"; }
+size_t lbm_config_bytes(void) { return sizeof(lbm_config_t); }
+const char* lbm_version(void) { return "paper_2506_17713_b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,384 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the oracle, element by element,
+on the same seeded inputs.  Gates (BASELINE.json north_star):
+  * integer work (link flags, boundary-solid list, pure streaming): bit-exact
+  * fp64 compute/store: max |df| <= 1e-11 after 100 steps
+  * fp32 compute: max |f32 - f64 oracle| / max |f64| <= 2e-5 after 100 steps
+  * fp16 storage: vs the fp32 oracle with emulated fp16 storage, max |df| <= 4 * 2^-11 * max |f|
+    
+Sizes span several thread blocks and have ragged tails (nx not a multiple of the block size).
+"""
+import numpy as np
+import pytest
+
+from conftest import make_oracle
+from paper_2506_17713_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-11
+TOL32 = 2e-5
+TOL16 = 4 * 2.0 ** -11
+
+
+def make_gpu(wl, inp):
+    from paper_2506_17713_b200 import binding
+    s = binding.LBM(wl)
+    if inp.get("mask") is not None:
+        s.set_solid_mask(inp["mask"])
+    dt = np.float32 if wl.get("compute_dtype", "f64") == "f32" else np.float64
+    s.init_fields([np.asarray(r, dtype=dt) for r in inp["rho"]], None if inp.get("u") is None else np.asarray(inp["u"], dtype=dt))
+    return s
+
+
+def with_dtype(wl, compute, store=None):
+    w = dict(wl)
+    w["compute_dtype"] = compute
+    w["store_dtype"] = store or compute
+    return w
+
+
+def run_pair(wl, inp, steps, oracle_wl=None):
+    o = make_oracle(oracle_wl or wl, inp)
+    g = make_gpu(wl, inp)
+    o.step(steps)
+    g.step(steps)
+    fo = [o.get_populations(k) for k in range(o.nc)]
+    fg = [g.get_populations(k) for k in range(g.nc)]
+    return o, g, fo, fg
+
+
+def fluid_mask(inp, N):
+    return np.ones(N, bool) if inp.get("mask") is None else (np.asarray(inp["mask"]).reshape(-1) == 0)
+
+
+def assert_parity(fo, fg, fluid, tol, relative):
+    for a, b in zip(fo, fg):
+        diff = np.abs(a[:, fluid] - b[:, fluid]).max()
+        scale = np.abs(a[:, fluid]).max() if relative else 1.0
+        assert np.isfinite(b).all()
+        assert diff <= tol * scale, (diff, scale)
+
+
+def small_inputs(wl, seed, lo=0.1, hi=0.2, mask=None):
+    N = wl["nx"] * wl["ny"] * wl["nz"]
+    rng = np.random.default_rng(seed)
+    rho = [lo + (hi - lo) * rng.uniform(size=N) for _ in range(wl["n_components"])]
+    if wl.get("compute_dtype") == "f32":
+        rho = [r.astype(np.float32).astype(np.float64) for r in rho]
+    return dict(rho=rho, u=None, mask=mask)
+
+
+# ------------------------------------------------------------------ the five configs at reduced size
+def test_config1_fp64_100_steps():
+    wl, inp = W.config1(64, "f64")
+    o, g, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    # macroscopic export (S8)
+    ro, uo, po = o.get_macroscopic()
+    rg, ug, pg = g.get_macroscopic()
+    assert np.abs(ro[0] - rg[0]).max() <= TOL64
+    assert np.abs(uo - ug).max() <= 1e-10
+    assert np.abs(po - pg).max() <= TOL64
+
+
+@pytest.mark.parametrize("nx,ny", [(70, 37), (200, 3), (1, 5)])
+def test_config1_ragged_sizes(nx, ny):
+    wl, _ = W.config1(8, "f64")
+    wl.update(nx=nx, ny=ny)
+    inp = small_inputs(wl, 11, 0.05, 0.25)
+    o, g, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+
+
+def test_config2_two_components_plates():
+    wl, inp = W.config2(96, 40, "f64", wall=3)
+    o, g, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    ro, uo, po = o.get_macroscopic()
+    rg, ug, pg = g.get_macroscopic()
+    for k in range(2):
+        assert np.abs(ro[k] - rg[k]).max() <= TOL64     # includes the virtual density at boundary solids
+    assert np.abs(uo - ug).max() <= 1e-10
+    # fp32 compute + store against the fp64 oracle
+    wl32, inp32 = W.config2(96, 40, "f32", wall=3)
+    o, g, fo, fg = run_pair(wl32, inp32, 100, oracle_wl=with_dtype(wl32, "f64"))
+    assert_parity(fo, fg, fluid_mask(inp32, o.N), TOL32, relative=True)
+
+
+def test_config3_mrt_peng_robinson():
+    wl, inp = W.config3(20, "f64")
+    wl.update(nx=22, ny=19, nz=17)
+    inp = small_inputs(wl, 3, 3.9, 4.2)
+    o, g, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    wl32 = with_dtype(wl, "f32")
+    inp32 = small_inputs(wl32, 3, 3.9, 4.2)
+    o, g, fo, fg = run_pair(wl32, inp32, 100, oracle_wl=wl)
+    # spinodal growth amplifies rounding differences (SURVEY 8(c) caveat): also compare with the fp32 oracle
+    o32 = make_oracle(wl32, inp32)
+    o32.step(100)
+    f32o = [o32.get_populations(0)]
+    d_gpu = np.abs(fg[0] - fo[0]).max() / np.abs(fo[0]).max()
+    d_cpu = np.abs(f32o[0] - fo[0]).max() / np.abs(fo[0]).max()
+    assert d_gpu <= max(TOL32, 3 * d_cpu), (d_gpu, d_cpu)
+
+
+@pytest.mark.parametrize("store", ["f64", "f32"])
+def test_config4_porous_inlet_outlet(store):
+    n = 36
+    wl, inp = W.config4(n, store_dtype="f32")
+    compute = "f64" if store == "f64" else "f32"
+    wl = with_dtype(wl, compute, store)
+    if compute == "f64":
+        o, g, fo, fg = run_pair(wl, inp, 100)
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+        ro, uo, po = o.get_macroscopic()
+        rg, ug, pg = g.get_macroscopic()
+        for k in range(2):
+            assert np.abs(ro[k] - rg[k]).max() <= TOL64
+        assert np.abs(uo - ug).max() <= 1e-10
+        assert np.abs(po - pg).max() <= TOL64
+    else:
+        o, g, fo, fg = run_pair(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL32, relative=True)
+
+
+def test_config4_fp16_storage():
+    n = 36
+    wl, inp = W.config4(n, store_dtype="f16")
+    o, g, fo, fg = run_pair(wl, inp, 100)      # oracle: fp32 compute with emulated fp16 storage
+    fl = fluid_mask(inp, o.N)
+    for a, b in zip(fo, fg):
+        assert np.abs(a[:, fl] - b[:, fl]).max() <= TOL16 * np.abs(a[:, fl]).max()
+    # one step from identical stored values must agree to fp32 rounding + at most one fp16 ulp flip
+    o = make_oracle(wl, inp)
+    g = make_gpu(wl, inp)
+    assert np.array_equal(o.get_populations(0), g.get_populations(0))   # fp16-rounded f_eq identical
+    o.step(1)
+    g.step(1)
+    a, b = o.get_populations(0)[:, fl], g.get_populations(0)[:, fl]
+    assert np.abs(a - b).max() <= 2.0 ** -10 * np.abs(a).max()
+    assert (a != b).mean() < 0.02
+
+
+@pytest.mark.parametrize("n,dtype", [(40, "f64"), (40, "f32")])
+def test_config5_droplets(n, dtype):
+    wl, inp = W.config5(n, dtype)
+    if dtype == "f64":
+        o, g, fo, fg = run_pair(wl, inp, 100)
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    else:
+        o, g, fo, fg = run_pair(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL32, relative=True)
+
+
+def test_paper_benchmark_exp_psi():
+    wl, inp = W.paper_benchmark(32, "f32")
+    o, g, fo, fg = run_pair(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL32, relative=True)
+
+
+# ------------------------------------------------------------------ other options of the path
+@pytest.mark.parametrize("lattice,n", [("D2Q9", (45, 23, 1)), ("D3Q19", (21, 10, 9))])
+@pytest.mark.parametrize("collision", ["BGK", "MRT"])
+@pytest.mark.parametrize("forcing", ["EDM", "SHIFT"])
+def test_collision_and_forcing_variants(lattice, n, collision, forcing):
+    tau = 0.8
+    wl = dict(lattice=lattice, nx=n[0], ny=n[1], nz=n[2], n_components=1, periodic=(True, True, True),
+              psi_kind=["CS"], eos=[dict(a=W.CS_A, b=W.CS_B, R=W.CS_R, T=W.CS_T_085)], G=[[-1.0]],
+              collision=collision, tau=[tau], forcing=forcing, compute_dtype="f64", store_dtype="f64")
+    if collision == "MRT":
+        rates = W.mrt_rates(lattice, tau)
+        if forcing == "SHIFT":   # momentum rows must relax at s_nu for the shifted equilibrium to inject F
+            for r in ([3, 5] if lattice == "D2Q9" else [3, 5, 7]):
+                rates[r] = 1.0 / tau
+        wl["mrt_rates"] = [rates]
+    inp = small_inputs(wl, 5, 0.1, 0.2)
+    o, g, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+
+
+@pytest.mark.parametrize("kind,eos", [
+    ("PR", dict(a=W.PR_A, b=W.PR_B, R=1.0, omega=W.PR_OMEGA, T=0.9 * 0.0729, alpha=0.5)),
+    ("VDW", dict(a=9 / 49, b=2 / 21, R=1.0, T=0.9 * 0.5714)),
+    ("RK", dict(a=2 / 49, b=2 / 21, R=1.0, T=0.9 * 0.1961)),
+    ("RKS", dict(a=2 / 49, b=2 / 21, R=1.0, omega=0.344, T=0.9 * 0.08686)),
+    ("EXP", dict()), ("RHO", dict()), ("SC93", dict(rho0=1.5)),
+])
+def test_every_pseudopotential_kind(kind, eos):
+    g = {"EXP": -10 / 3, "RHO": -0.05, "SC93": -1.2}.get(kind, -1.0)
+    lo, hi = (2.0, 4.0) if kind in ("PR", "VDW", "RK", "RKS") else (0.5, 1.5)
+    wl = dict(lattice="D2Q9", nx=50, ny=20, nz=1, n_components=1, periodic=(True, True, True),
+              psi_kind=[kind], eos=[eos], G=[[g]], collision="BGK", tau=[1.0], forcing="EDM",
+              compute_dtype="f64", store_dtype="f64")
+    inp = small_inputs(wl, 6, lo, hi)
+    o, gp, fo, fg = run_pair(wl, inp, 50)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    assert np.abs(o.get_psi(0) - gp.get_psi(0)).max() <= 1e-13
+
+
+def test_two_components_different_tau_and_intra_coupling():
+    g = 0.57
+    wl = dict(lattice="D3Q19", nx=18, ny=11, nz=10, n_components=2, periodic=(True, True, True),
+              psi_kind=["RHO", "RHO"], eos=[dict(), dict()], G=[[-0.027, g], [g, -0.027]],
+              collision="BGK", tau=[1.0, 0.7], forcing="EDM", compute_dtype="f64", store_dtype="f64")
+    inp = small_inputs(wl, 7, 0.3, 0.7)
+    o, gp, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+
+
+def test_rho_ref_shifted_storage_fp16():
+    wl, inp = W.config5(24, "f32", store_dtype="f16")
+    wl["rho_ref"] = 0.15
+    o, g, fo, fg = run_pair(wl, inp, 50)
+    for a, b in zip(fo, fg):
+        assert np.abs(a - b).max() <= TOL16 * np.abs(a).max()
+
+
+# ------------------------------------------------------------------ integer / bit-exact work
+def _random_mask(n, frac, seed):
+    rng = np.random.default_rng(seed)
+    return (rng.uniform(size=n[0] * n[1] * n[2]) < frac).astype(np.uint8)
+
+
+@pytest.mark.parametrize("lattice,n,periodic", [
+    ("D2Q9", (67, 33, 1), (True, True, True)),
+    ("D2Q9", (67, 33, 1), (False, True, True)),
+    ("D3Q19", (19, 17, 13), (True, True, True)),
+    ("D3Q19", (19, 17, 13), (False, False, True)),
+])
+def test_link_flags_and_boundary_solids_bit_exact(lattice, n, periodic):
+    from oracle import lbm_oracle as orc
+    from paper_2506_17713_b200 import binding
+    wl = dict(lattice=lattice, nx=n[0], ny=n[1], nz=n[2], n_components=1, periodic=periodic, psi_kind=["RHO"],
+              eos=[dict()], G=[[0.0]], collision="BGK", tau=[1.0], forcing="EDM", compute_dtype="f32",
+              store_dtype="f32")
+    mask = _random_mask(n, 0.35, 21)
+    o = orc.Oracle(wl)
+    o.set_solid_mask(mask)
+    g = binding.LBM(wl)
+    g.set_solid_mask(mask)
+    assert np.array_equal(o.get_link_flags(), g.get_link_flags())
+    assert np.array_equal(o.get_boundary_solids(), g.get_boundary_solids())
+    # no mask at all
+    g2 = binding.LBM(wl)
+    o2 = orc.Oracle(wl)
+    assert np.array_equal(o2.get_link_flags(), g2.get_link_flags())
+    assert g2.get_boundary_solids().size == 0
+
+
+@pytest.mark.parametrize("lattice,n,periodic,dtype", [
+    ("D2Q9", (37, 21, 1), (True, True, True), "f64"),
+    ("D3Q19", (13, 11, 7), (True, True, True), "f32"),
+    ("D3Q19", (13, 11, 7), (False, True, False), "f64"),
+])
+@pytest.mark.parametrize("with_mask", [False, True])
+def test_pure_streaming_bit_exact(lattice, n, periodic, dtype, with_mask):
+    """NO_COLLIDE: populations are only moved (and bounced); the GPU must equal the oracle bit for bit."""
+    from oracle import lbm_oracle as orc
+    from paper_2506_17713_b200 import binding
+    q = 9 if lattice == "D2Q9" else 19
+    N = n[0] * n[1] * n[2]
+    wl = dict(lattice=lattice, nx=n[0], ny=n[1], nz=n[2], n_components=1, periodic=periodic, psi_kind=["RHO"],
+              eos=[dict()], G=[[0.0]], collision="BGK", tau=[1.0], forcing="EDM", compute_dtype=dtype,
+              store_dtype=dtype, no_collide=True)
+    mask = _random_mask(n, 0.2, 22) if with_mask else None
+    rng = np.random.default_rng(23)
+    f0 = rng.uniform(0.1, 1.0, size=(q, N))
+    if dtype == "f32":
+        f0 = f0.astype(np.float32).astype(np.float64)
+    o = orc.Oracle(wl)
+    g = binding.LBM(wl)
+    if with_mask:
+        o.set_solid_mask(mask)
+        g.set_solid_mask(mask)
+    o.init_fields([np.ones(N)])
+    g.init_fields([np.ones(N, dtype=np.float32 if dtype == "f32" else np.float64)])
+    o.set_populations(0, f0)
+    g.set_populations(0, f0)
+    assert np.array_equal(o.get_populations(0), g.get_populations(0))
+    for steps in (1, 2, 5):
+        o.step(steps)
+        g.step(steps)
+        assert np.array_equal(o.get_populations(0), g.get_populations(0))
+    if mask is None and all(periodic):
+        left = int(np.lcm.reduce(n)) - 8
+        g.step(left)
+        assert np.array_equal(g.get_populations(0), f0)   # the permutation returns to the start
+
+
+# ------------------------------------------------------------------ physics-level agreement
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_coexistence_densities_match_oracle(dtype):
+    """Flat interface, CS T_r = 0.85: equilibrium liquid / vapour densities agree with the fp64 oracle to 1e-4."""
+    nx, ny = 128, 2
+    x = np.tile(np.arange(nx), ny).astype(float)
+    rho0 = W.tanh_profile(np.abs(x - (nx - 1) / 2), nx / 4, 3.0, W.CS_RHO_L_085, W.CS_RHO_V_085)
+    wl = dict(lattice="D2Q9", nx=nx, ny=ny, nz=1, n_components=1, periodic=(True, True, True), psi_kind=["CS"],
+              eos=[dict(a=W.CS_A, b=W.CS_B, R=W.CS_R, T=W.CS_T_085)], G=[[-1.0]], collision="BGK", tau=[1.0],
+              forcing="EDM", compute_dtype=dtype, store_dtype=dtype)
+    if dtype == "f32":
+        rho0 = rho0.astype(np.float32).astype(np.float64)
+    inp = dict(rho=[rho0], u=None, mask=None)
+    o = make_oracle(with_dtype(wl, "f64"), inp)
+    g = make_gpu(wl, inp)
+    o.step(6000)
+    g.step(6000)
+    ro = o.get_macroscopic()[0][0].reshape(ny, nx)[0]
+    rg = g.get_macroscopic()[0][0].reshape(ny, nx)[0]
+    assert abs(rg[nx // 2] - ro[nx // 2]) <= 1e-4
+    assert abs(rg[0] - ro[0]) <= 1e-4
+    m0 = rho0.sum()
+    assert abs(g.get_populations(0).sum() - m0) <= (1e-11 if dtype == "f64" else 2e-5) * m0
+
+
+# ------------------------------------------------------------------ API behaviour
+def test_api_state_and_errors():
+    import ctypes as C
+    from paper_2506_17713_b200 import binding
+    wl, inp = W.config1(16, "f64")
+    g = binding.LBM(wl)
+    assert g.L.lbm_step(g.h, 1) == -5                       # LBM_E_STATE: step before init
+    assert b"before" in g.L.lbm_last_error(g.h)
+    assert g.L.lbm_step(g.h, -1) == -1
+    g.init_fields(inp["rho"])
+    assert g.L.lbm_set_solid_mask(g.h, inp["rho"][0].ctypes.data_as(C.c_void_p), 0) == -5   # mask after init
+    assert g.L.lbm_set_face_bc(g.h, 0, 1, None, None) == -1  # periodic axis
+    f0 = g.get_populations(0)
+    g.step(0)
+    assert g.steps_done == 0 and np.array_equal(g.get_populations(0), f0)
+    g.step(3)
+    assert g.steps_done == 3 and g.kernel_launches >= 6
+    # workspace too small / misaligned
+    import torch
+    cfg = binding.make_config(wl)
+    need = g.L.lbm_workspace_bytes(C.byref(cfg))
+    ws = torch.empty(need + 256, dtype=torch.uint8, device="cuda")
+    h = C.c_void_p()
+    assert g.L.lbm_create(C.byref(cfg), C.c_void_p(ws.data_ptr()), need - 1, None, C.byref(h)) == -3
+    assert g.L.lbm_create(C.byref(cfg), C.c_void_p(ws.data_ptr() + 8), need, None, C.byref(h)) == -3
+    host = np.zeros(16, dtype=np.uint8)
+    assert g.L.lbm_create(C.byref(cfg), host.ctypes.data_as(C.c_void_p), need, None, C.byref(h)) in (-1, -3)
+
+
+def test_device_resident_io_and_reinit():
+    import torch
+    from paper_2506_17713_b200 import binding
+    wl, inp = W.config5(24, "f32")
+    g = binding.LBM(wl)
+    rho_dev = torch.from_numpy(inp["rho"][0].astype(np.float32)).cuda()
+    g.init_fields([rho_dev])
+    g.step(10)
+    rho, u, p = g.get_macroscopic_device()
+    f_dev = g.get_populations_device(0)
+    o = make_oracle(with_dtype(wl, "f64"), inp)
+    o.step(10)
+    assert np.abs(f_dev.cpu().numpy() - o.get_populations(0)).max() <= TOL32 * np.abs(o.get_populations(0)).max()
+    ro, uo, po = o.get_macroscopic()
+    assert np.abs(rho[0].cpu().numpy() - ro[0]).max() <= 1e-5
+    assert np.abs(u.cpu().numpy() - uo).max() <= 1e-5
+    # re-initialisation restarts the run
+    g.init_fields([rho_dev])
+    assert g.steps_done == 0
+    g.step(10)
+    assert torch.equal(g.get_populations_device(0), f_dev)
