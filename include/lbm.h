@@ -175,6 +175,22 @@ LBM_API int lbm_get_lattice(int lattice, int* q, int* e, double* w, int* opposit
 /* sizeof(lbm_config_t) as compiled into the library (ABI check for bindings). */
 LBM_API size_t lbm_config_bytes(void);
 
+/* Measurement only: per-kernel device time of the hot loop.  While enabled, lbm_step brackets each of its
+ * kernels with a pair of CUDA events recorded on the handle's stream (this serialises nothing but adds two
+ * event records per kernel, so whole-step throughput is measured with profiling OFF).
+ * lbm_get_kernel_times synchronises the stream, adds up the elapsed time of every bracketed launch since the
+ * last call and resets the accumulators.  ms_total / launches: host arrays of LBM_K_COUNT entries indexed by
+ * lbm_kernel_id.  Errors: LBM_E_INVALID, LBM_E_CUDA. */
+enum lbm_kernel_id {
+    LBM_K_MOMENTS = 0, /* K1: rho + psi (two-pass path) */
+    LBM_K_VIRTUAL = 1, /* K1b: virtual density at boundary solids */
+    LBM_K_STEP = 2,    /* K2: fused stream + force + collide + boundary (two-pass path) */
+    LBM_K_FUSED = 3,   /* K2F: one-pass kernel (moments + psi of the halo recomputed in the tile) */
+    LBM_K_COUNT = 4
+};
+LBM_API int lbm_set_profiling(lbm_t* h, int enable);
+LBM_API int lbm_get_kernel_times(lbm_t* h, double* ms_total, int64_t* launches);
+
 /* Bookkeeping. */
 LBM_API int64_t lbm_steps_done(const lbm_t* h);
 LBM_API int64_t lbm_kernel_launches(const lbm_t* h); /* kernels launched by this handle so far */

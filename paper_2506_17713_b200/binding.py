@@ -25,6 +25,7 @@ COLLISIONS = {"BGK": 0, "MRT": 1}
 FORCINGS = {"EDM": 0, "SHIFT": 1}
 DTYPES = {"f16": 0, "f32": 1, "f64": 2}
 FACE_KINDS = {"PERIODIC": 0, "WALL": 1, "VELOCITY": 2, "PRESSURE": 3}
+KERNEL_IDS = {"moments": 0, "virtual": 1, "step": 2, "fused": 3}
 FLAG_NO_COLLIDE = 1
 STATUS = {0: "LBM_OK", -1: "LBM_E_INVALID", -2: "LBM_E_UNSUPPORTED", -3: "LBM_E_NOMEM", -4: "LBM_E_CUDA",
           -5: "LBM_E_STATE"}
@@ -71,6 +72,8 @@ _SIGNATURES = {
     "lbm_get_boundary_solids": (C.c_int64, [C.c_void_p, C.c_void_p, C.c_int64]),
     "lbm_get_psi": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int]),
     "lbm_get_lattice": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "lbm_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
+    "lbm_get_kernel_times": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "lbm_steps_done": (C.c_int64, [C.c_void_p]),
     "lbm_kernel_launches": (C.c_int64, [C.c_void_p]),
     "lbm_last_error": (C.c_char_p, [C.c_void_p]),
@@ -318,6 +321,16 @@ class LBM:
         out = np.empty(self.N, dtype=dtype)
         self._check(self.L.lbm_get_psi(self.h, k, out.ctypes.data_as(C.c_void_p), code, 0), "lbm_get_psi")
         return out
+
+    def set_profiling(self, enable: bool):
+        self._check(self.L.lbm_set_profiling(self.h, 1 if enable else 0), "lbm_set_profiling")
+
+    def get_kernel_times(self):
+        """{kernel name: (total ms, launches)} since the last call (measurement only)."""
+        ms = (C.c_double * len(KERNEL_IDS))()
+        cnt = (C.c_int64 * len(KERNEL_IDS))()
+        self._check(self.L.lbm_get_kernel_times(self.h, ms, cnt), "lbm_get_kernel_times")
+        return {name: (ms[i], int(cnt[i])) for name, i in KERNEL_IDS.items()}
 
     @property
     def steps_done(self) -> int:

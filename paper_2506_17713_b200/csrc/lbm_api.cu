@@ -44,6 +44,13 @@ struct lbm {
     double face_rho[6][2], face_u[6][3];
     int64_t steps, launches;
     std::string err;
+    // measurement only (lbm_set_profiling): event pairs around hot-loop kernels
+    bool profiling;
+    std::vector<cudaEvent_t> ev_pool;
+    struct EvPair { int kid; cudaEvent_t a, b; };
+    std::vector<EvPair> ev_pending;
+    double k_ms[LBM_K_COUNT];
+    int64_t k_cnt[LBM_K_COUNT];
 };
 
 namespace {
@@ -277,9 +284,54 @@ launch_fn pick_launch(const lbm_config_t& c) {
     return nullptr;
 }
 
+// ---- measurement only: event brackets around hot-loop kernels
+int prof_drain(lbm* h) {
+    if (h->ev_pending.empty()) return LBM_OK;
+    CU(cudaStreamSynchronize(h->stream));
+    for (auto& pr : h->ev_pending) {
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, pr.a, pr.b));
+        h->k_ms[pr.kid] += ms;
+        h->k_cnt[pr.kid] += 1;
+        h->ev_pool.push_back(pr.a);
+        h->ev_pool.push_back(pr.b);
+    }
+    h->ev_pending.clear();
+    return LBM_OK;
+}
+int prof_event(lbm* h, cudaEvent_t* ev) {
+    if (h->ev_pool.empty()) {
+        CU(cudaEventCreate(ev));
+    } else {
+        *ev = h->ev_pool.back();
+        h->ev_pool.pop_back();
+    }
+    CU(cudaEventRecord(*ev, h->stream));
+    return LBM_OK;
+}
+
+int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, int in_buf, int out_buf);
+
+// hot-loop launch, bracketed by events while profiling is on
+int hot_launch(lbm* h, int op, int kid) {
+    if (!h->profiling) return do_launch(h, op, nullptr, nullptr, nullptr, 0, -1, -1);
+    if (h->ev_pending.size() >= 2048) { int rc = prof_drain(h); if (rc) return rc; }
+    lbm::EvPair pr;
+    pr.kid = kid;
+    int rc = prof_event(h, &pr.a);
+    if (rc) return rc;
+    rc = do_launch(h, op, nullptr, nullptr, nullptr, 0, -1, -1);
+    if (rc) return rc;
+    rc = prof_event(h, &pr.b);
+    if (rc) return rc;
+    h->ev_pending.push_back(pr);
+    return LBM_OK;
+}
+
 // in_buf / out_buf: which population buffer the kernel reads / writes (-1 = current / the other one)
 int do_launch(lbm* h, int op, const void* a0 = nullptr, const void* a1 = nullptr, void* a2 = nullptr, int i0 = 0,
-              int in_buf = -1, int out_buf = -1) {
+              int in_buf = -1, int out_buf = -1);
+int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, int in_buf, int out_buf) {
     if (in_buf < 0) in_buf = h->cur;
     if (out_buf < 0) out_buf = h->cur ^ 1;
     LaunchArgs a;
@@ -449,6 +501,8 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->nbsolid = 0;
     h->steps = 0;
     h->launches = 0;
+    h->profiling = false;
+    for (int k = 0; k < LBM_K_COUNT; ++k) { h->k_ms[k] = 0.0; h->k_cnt[k] = 0; }
     for (int f = 0; f < 6; ++f) {
         h->face_kind[f] = cfg->periodic[f / 2] ? LBM_FACE_PERIODIC : LBM_FACE_WALL;
         h->face_rho[f][0] = h->face_rho[f][1] = 1.0;
@@ -458,7 +512,32 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     return LBM_OK;
 }
 
-void lbm_destroy(lbm_t* h) { delete h; }
+void lbm_destroy(lbm_t* h) {
+    if (!h) return;
+    for (auto& pr : h->ev_pending) { cudaEventDestroy(pr.a); cudaEventDestroy(pr.b); }
+    for (auto e : h->ev_pool) cudaEventDestroy(e);
+    delete h;
+}
+
+int lbm_set_profiling(lbm_t* h, int enable) {
+    if (!h) return LBM_E_INVALID;
+    if (!enable) { int rc = prof_drain(h); if (rc) return rc; }
+    h->profiling = enable != 0;
+    return LBM_OK;
+}
+
+int lbm_get_kernel_times(lbm_t* h, double* ms_total, int64_t* launches) {
+    if (!h) return LBM_E_INVALID;
+    int rc = prof_drain(h);
+    if (rc) return rc;
+    for (int k = 0; k < LBM_K_COUNT; ++k) {
+        if (ms_total) ms_total[k] = h->k_ms[k];
+        if (launches) launches[k] = h->k_cnt[k];
+        h->k_ms[k] = 0.0;
+        h->k_cnt[k] = 0;
+    }
+    return LBM_OK;
+}
 
 int lbm_set_solid_mask(lbm_t* h, const uint8_t* mask, int on_device) {
     if (!h || !mask) return LBM_E_INVALID;
@@ -529,10 +608,10 @@ int lbm_step(lbm_t* h, int n) {
     if (rc) return rc;
     for (int s = 0; s < n; ++s) {
         if (!(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) {
-            if ((rc = do_launch(h, OP_MOMENTS))) return rc;
-            if (h->nbsolid > 0 && (rc = do_launch(h, OP_VIRTUAL))) return rc;
+            if ((rc = hot_launch(h, OP_MOMENTS, LBM_K_MOMENTS))) return rc;
+            if (h->nbsolid > 0 && (rc = hot_launch(h, OP_VIRTUAL, LBM_K_VIRTUAL))) return rc;
         }
-        if ((rc = do_launch(h, OP_STEP))) return rc;
+        if ((rc = hot_launch(h, OP_STEP, LBM_K_STEP))) return rc;
         h->cur ^= 1;
         h->local = 0;
         h->steps++;

@@ -123,8 +123,11 @@ def config3(n: int = 256, dtype: str = "f32", alpha: float = 0.5):
 # ---------------------------------------------------------------- config 4
 def sphere_pack_mask(nx, ny, nz, porosity=0.20, rmin=6.0, rmax=14.0, buffer=8, seed_no=4):
     """Seeded overlapping-sphere solid mask, periodic in y and z, solid-free buffers at both x ends;
-    pore cells not 6-connected to the inlet plane are filled.  Returns (mask uint8 [N], porosity)."""
+    pore cells not 6-connected (periodically in y, z) to the inlet plane are filled.
+    Returns (mask uint8 [N], porosity of the core x in [buffer, nx-buffer))."""
     from scipy import ndimage
+    from scipy.sparse import coo_matrix
+    from scipy.sparse.csgraph import connected_components
 
     r = _rng(seed_no, 1)
     solid = np.zeros((nz, ny, nx), dtype=bool)
@@ -133,9 +136,9 @@ def sphere_pack_mask(nx, ny, nz, porosity=0.20, rmin=6.0, rmax=14.0, buffer=8, s
     # radii scale with the box so that reduced-size tests keep several spheres
     scale = min(1.0, min(nx, ny, nz) / 100.0)
     rmin, rmax = max(2.0, rmin * scale), max(3.0, rmax * scale)
-    zz, yy, xx = np.ogrid[:nz, :ny, :nx]
+    npore = ncore          # pore cells of the core, tracked incrementally
     guard = 0
-    while (~solid[:, :, core]).sum() / ncore > porosity and guard < 200000:
+    while npore / ncore > porosity and guard < 2000000:
         guard += 1
         cx, cy, cz = r.uniform(0, nx), r.uniform(0, ny), r.uniform(0, nz)
         rad = r.uniform(rmin, rmax)
@@ -144,24 +147,37 @@ def sphere_pack_mask(nx, ny, nz, porosity=0.20, rmin=6.0, rmax=14.0, buffer=8, s
             continue
         ys = np.arange(int(np.floor(cy - rad)), int(np.ceil(cy + rad)) + 1)
         zs = np.arange(int(np.floor(cz - rad)), int(np.ceil(cz + rad)) + 1)
+        if len(ys) >= ny or len(zs) >= nz:   # tiny test boxes: a sphere may not wrap onto itself
+            continue
         xs = np.arange(x0, x1)
         d2 = ((zs[:, None, None] - cz) ** 2 + (ys[None, :, None] - cy) ** 2 + (xs[None, None, :] - cx) ** 2)
         ball = d2 <= rad * rad
-        solid[np.ix_(zs % nz, ys % ny, xs)] |= ball
-    # keep only pore space connected to the inlet plane (6-connectivity, periodic in y and z via padding)
+        ix = np.ix_(zs % nz, ys % ny, xs)
+        sub = solid[ix]
+        npore -= int((ball & ~sub).sum())
+        solid[ix] = sub | ball
+    # keep only the pore space connected to the inlet plane: label without wrap, then join labels that
+    # touch across the periodic y and z faces, and keep the groups that reach x = 0
     pore = ~solid
-    tiled = np.tile(pore, (3, 3, 1))
-    lab, _ = ndimage.label(tiled)
-    centre = lab[nz:2 * nz, ny:2 * ny, :]
-    inlet_labels = np.unique(centre[:, :, 0])
-    inlet_labels = inlet_labels[inlet_labels > 0]
-    connected = np.isin(lab, inlet_labels)
-    # a pore cell is kept if any of its periodic images is connected to an inlet image
-    keep = np.zeros_like(pore)
-    for iz in range(3):
-        for iy in range(3):
-            keep |= connected[iz * nz:(iz + 1) * nz, iy * ny:(iy + 1) * ny, :]
-    solid = ~(pore & keep)
+    lab, nlab = ndimage.label(pore)
+    pairs = []
+    for a_, b_ in ((lab[0, :, :], lab[-1, :, :]), (lab[:, 0, :], lab[:, -1, :])):
+        both = (a_ > 0) & (b_ > 0)
+        if both.any():
+            pairs.append(np.unique(np.stack([a_[both], b_[both]], axis=1), axis=0))
+    if pairs:
+        pr = np.concatenate(pairs, axis=0)
+        g = coo_matrix((np.ones(len(pr), dtype=np.int8), (pr[:, 0], pr[:, 1])), shape=(nlab + 1, nlab + 1))
+        _, group = connected_components(g, directed=False)
+    else:
+        group = np.arange(nlab + 1)
+    inlet = np.unique(lab[:, :, 0])
+    inlet = inlet[inlet > 0]
+    keep_group = np.zeros(group.max() + 1, dtype=bool)
+    keep_group[group[inlet]] = True
+    keep_label = keep_group[group]
+    keep_label[0] = False
+    solid = ~keep_label[lab]
     por = float((~solid[:, :, core]).sum() / ncore)
     return solid.astype(np.uint8).reshape(-1), por
 
@@ -180,7 +196,8 @@ def config4(n: int = 400, store_dtype: str = "f16", drho_nw: float = 0.5, buffer
         face_bc={0: ("VELOCITY", (1.0, 0.03), (1e-3, 0.0, 0.0)), 1: ("PRESSURE", (0.03, 1.0), (0.0, 0.0, 0.0))},
     )
     mask, por = sphere_pack_mask(n, n, n, porosity=0.20, buffer=buffer)
-    wl["porosity"] = por
+    wl["porosity"] = por                                  # of the core x in [buffer, n-buffer)
+    wl["fluid_fraction"] = float(1.0 - mask.mean())       # of the whole box
     x, _, _ = _grid(n, n, n)
     nw = np.where(x < buffer, 1.0, 0.03)
     w = np.where(x < buffer, 0.03, 1.0)
