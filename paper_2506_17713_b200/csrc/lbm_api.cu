@@ -37,7 +37,7 @@ struct lbm {
     char* ws;
     Carve cv;
     int cur;
-    int local;
+    int vec;   // cells per thread in the hot kernels (1 or the dtype's vector width)
     bool initialized, has_solid, bnd, dirty, force_rho;
     int nbsolid;
     int face_kind[6];
@@ -122,6 +122,31 @@ void lattice_weights(double* w) {
     for (int i = 0; i < L::Q; ++i) w[i] = (double)L::WN[i] / (double)L::WD;
 }
 
+// M^-1 S M = sum_r (s_r / |M_r|^2) M_r^T M_r split by the parity of the moment polynomial of row r (R9):
+// even rows act on (f_0, f_a + f_b) only, odd rows on (f_a - f_b) only (a = 2p+1, b = 2p+2).
+//   ce[P][Q] = sum_{r even} c_r M_r,i(P) M_r,i(Q),  i(0) = 0, i(P) = 2P-1;   co[P][Q] = sum_{r odd} c_r M_r,2P+1 M_r,2Q+1
+template <class L>
+void mrt_blocks(const double* rates, double (&ce)[10][10], double (&co)[9][9]) {
+    constexpr int NP = (L::Q - 1) / 2;
+    for (auto& row : ce) for (double& v : row) v = 0.0;
+    for (auto& row : co) for (double& v : row) v = 0.0;
+    for (int r = 0; r < L::Q; ++r) {
+        double m[19], n2 = 0.0;
+        for (int i = 0; i < L::Q; ++i) { m[i] = 0.5 * mrt_entry2<L>(r, i); n2 += m[i] * m[i]; }
+        bool even = true;
+        for (int pq = 0; pq < NP; ++pq)
+            if (m[2 * pq + 1] != m[2 * pq + 2]) even = false;
+        const double cr = rates[r] / n2;
+        if (even) {
+            for (int P = 0; P <= NP; ++P)
+                for (int Q = 0; Q <= NP; ++Q) ce[P][Q] += cr * m[P ? 2 * P - 1 : 0] * m[Q ? 2 * Q - 1 : 0];
+        } else {
+            for (int P = 0; P < NP; ++P)
+                for (int Q = 0; Q < NP; ++Q) co[P][Q] += cr * m[2 * P + 1] * m[2 * Q + 1];
+        }
+    }
+}
+
 template <class CT>
 KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
     KParams<CT> p;
@@ -137,8 +162,6 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
     p.flags = reinterpret_cast<const uint32_t*>(h->ws + h->cv.flags);
     p.bsolid = reinterpret_cast<const int*>(h->ws + h->cv.bsolid);
     p.nbsolid = h->nbsolid;
-    p.local = h->local;
-    p.no_collide = (c.flags & LBM_FLAG_NO_COLLIDE) ? 1 : 0;
     p.forcing = c.forcing == LBM_SHIFT ? 1 : 0;
     p.write_rho = (h->nbsolid > 0 || h->force_rho) ? 1 : 0;
     double w[19];
@@ -149,7 +172,21 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
         p.tau[k] = (CT)c.tau[k];
         p.inv_tau[k] = (CT)(1.0 / c.tau[k]);
         for (int kp = 0; kp < c.n_components; ++kp) p.G[k][kp] = (CT)c.G[k][kp];
-        for (int r = 0; r < h->q; ++r) p.mrt_s[k][r] = (CT)c.mrt_rates[k][r];
+        // BGK as one linear combination (lbm_hot.cuh collide): EDM  f* = (1-w) f + (w-1) feq(u') + feq(u'+du),
+        // SHIFT  f* = (1-w) f + w feq(u' + tau du), w = 1/tau
+        const double om = 1.0 / c.tau[k];
+        p.c_keep[k] = (CT)(1.0 - om);
+        p.c_feq_a[k] = (CT)(c.forcing == LBM_SHIFT ? om : om - 1.0);
+        p.c_feq_b[k] = (CT)(c.forcing == LBM_SHIFT ? 0.0 : 1.0);
+        if (c.collision == LBM_MRT) {
+            double ce[10][10], co[9][9];
+            if (c.lattice == LBM_D2Q9) mrt_blocks<D2Q9>(c.mrt_rates[k], ce, co);
+            else mrt_blocks<D3Q19>(c.mrt_rates[k], ce, co);
+            for (int r = 0; r < 10; ++r)
+                for (int q2 = 0; q2 < 10; ++q2) p.mrt_ce[k][r][q2] = (CT)ce[r][q2];
+            for (int r = 0; r < 9; ++r)
+                for (int q2 = 0; q2 < 9; ++q2) p.mrt_co[k][r][q2] = (CT)co[r][q2];
+        }
         const lbm_eos_t& e = c.eos[k];
         p.psi_kind[k] = e.psi_kind;
         p.eos_a[k] = (CT)e.a;
@@ -337,8 +374,9 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     LaunchArgs a;
     a.op = op;
     a.nc = h->cfg.n_components;
-    a.coll = h->cfg.collision == LBM_MRT ? 1 : 0;
+    a.coll = (h->cfg.flags & LBM_FLAG_NO_COLLIDE) ? 2 : (h->cfg.collision == LBM_MRT ? 1 : 0);
     a.bnd = h->bnd ? 1 : 0;
+    a.vec = h->vec;
     a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
     a.stream = h->stream;
     launch_fn fn = pick_launch(h->cfg);
@@ -492,7 +530,15 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->ws = static_cast<char*>(d_workspace);
     h->cv = cv;
     h->cur = 0;
-    h->local = 1;
+    h->vec = 1;
+    {   // widest vector the hot kernels were built with for this dtype / component count, if nx allows it
+        const int sb = (int)h->sbytes, cb = (int)h->cbytes;
+        int v = 16 / sb;
+        const int cap = 4 / (cfg->n_components * (cb / 4));
+        if (v > cap) v = cap;
+        if (v < 1) v = 1;
+        if (cfg->nx % v == 0) h->vec = v;
+    }
     h->initialized = false;
     h->has_solid = false;
     h->dirty = true;
@@ -590,12 +636,13 @@ int lbm_init_fields(lbm_t* h, const void* const* rho, const void* u, int dtype, 
             for (int a = 0; a < h->d; ++a)
                 if ((rc = stage(2 + a, static_cast<const char*>(u) + ((size_t)a * h->N + c0) * eb, &io.in[2 + a])))
                     return rc;
-        // fill the CURRENT buffer; solid cells are written to the other buffer too
+        // post-stream f(x,0) into BOTH buffers
         rc = do_launch(h, OP_INIT, &io, nullptr, h->ws + h->cv.f[h->cur ^ 1], h->bnd ? 1 : 0, h->cur ^ 1, h->cur);
         if (rc) return rc;
         if (!on_device) CU(cudaStreamSynchronize(h->stream));  // staging slots are reused by the next chunk
     }
-    h->local = 1;
+    // scatter into the storage convention of the hot loop: read buffer cur^1, write buffer cur
+    if ((rc = do_launch(h, OP_UNSTREAM, nullptr, nullptr, nullptr, -1, h->cur ^ 1, h->cur))) return rc;
     h->steps = 0;
     h->initialized = true;
     return LBM_OK;
@@ -613,7 +660,6 @@ int lbm_step(lbm_t* h, int n) {
         }
         if ((rc = hot_launch(h, OP_STEP, LBM_K_STEP))) return rc;
         h->cur ^= 1;
-        h->local = 0;
         h->steps++;
     }
     return LBM_OK;
@@ -701,7 +747,7 @@ int lbm_set_populations(lbm_t* h, int comp, const void* f, int dtype, int on_dev
     if (comp < 0 || comp >= h->cfg.n_components) return fail(h, LBM_E_INVALID, "component");
     if (dtype != LBM_F32 && dtype != LBM_F64) return fail(h, LBM_E_INVALID, "dtype");
     if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_set_populations before lbm_init_fields");
-    if (!h->local) return fail(h, LBM_E_STATE, "lbm_set_populations is only valid right after lbm_init_fields");
+    if (h->steps != 0) return fail(h, LBM_E_STATE, "lbm_set_populations is only valid right after lbm_init_fields");
     int rc = prepare(h);
     if (rc) return rc;
     const size_t eb = dtype_bytes(dtype);
@@ -721,7 +767,8 @@ int lbm_set_populations(lbm_t* h, int comp, const void* f, int dtype, int on_dev
         if (rc) return rc;
         if (!on_device) CU(cudaStreamSynchronize(h->stream));
     }
-    return LBM_OK;
+    // both buffers now hold the post-stream values of this component: scatter cur^1 -> cur (storage convention)
+    return do_launch(h, OP_UNSTREAM, nullptr, nullptr, nullptr, comp, h->cur ^ 1, h->cur);
 }
 
 int lbm_get_link_flags(lbm_t* h, uint32_t* flags, int on_device) {

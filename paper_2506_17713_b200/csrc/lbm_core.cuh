@@ -1,20 +1,21 @@
 // lbm_core.cuh -- device code of the Shan-Chen LBM step for sm_100a.
 //
 // Kernels (SURVEY.md section 8(a) step numbers; paper citations P:<line> = PAPER.md line):
-//   k_moments          K1   S1 (rho only) + S3: rho^k = sum_i f_i^k (Eq. 4/10), psi^k (Eq. 12)
+//   k_moments_v        K1   (lbm_hot.cuh) S1 (rho only) + S3: rho^k = sum_i f_i^k (Eq. 4/10), psi^k (Eq. 12)
 //   k_virtual_density  K1b  S2 (+S3 there): improved virtual density at boundary solids (Eq. 17)
-//   k_step             K2   S1 (j) + S4..S7 fused: pull-stream, force (Eq. 13), common velocity,
-//                           BGK/MRT collision (Eq. 3), EDM / shift forcing (Eq. 5),
+//   k_step_v           K2   (lbm_hot.cuh) S1 (j) + S4..S7 fused: pull-stream, force (Eq. 13), common
+//                           velocity, BGK/MRT collision (Eq. 3), EDM / shift forcing (Eq. 5),
 //                           halfway bounce-back and inlet/outlet faces
-//   k_init, k_export_* S0 and S8, off the hot loop.
+//   k_init, k_unstream, k_export_*, k_import_pop   S0 and S8, off the hot loop (this file).
 //
 // Storage: populations are SoA planes [component][direction][cell], x fastest, in the storage
 // dtype ST; arithmetic is in the compute dtype CT.  Between steps the planes hold the POST-COLLISION
 // populations f*_i(x,t) with every boundary rule already applied at the writing cell, so that the
 // pull of the next step is pure indexing: f_i(x,t+1) = stored_i(x - e_i), or stored_ibar(x) when the
-// link flag of direction i is set (source solid / beyond a non-periodic face).  Right after
-// lbm_init_fields / lbm_set_populations the planes hold post-stream values and the first step reads
-// them in place (`local` = 1).
+// link flag of direction i is set (source solid / beyond a non-periodic face).  lbm_init_fields /
+// lbm_set_populations produce post-stream values f(x,0); k_unstream scatters them once into this
+// storage convention (stored_i(x - e_i) = f_i(x), or stored_ibar(x) = f_i(x) on a flagged link), so the
+// hot kernels never see a special first step.
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
@@ -133,14 +134,14 @@ struct KParams {
     const int* bsolid; // boundary-solid list
     int nbsolid;
     // mode
-    int local;         // planes hold post-stream values (first step after init): read in place
-    int no_collide;
     int forcing;       // 0 EDM, 1 SHIFT
     int write_rho;     // K1 also writes rho (needed by K1b and the exports)
     // physics
     CT tau[2], inv_tau[2];
     CT G[2][2];
-    CT mrt_s[2][19];
+    CT mrt_ce[2][10][10];  // MRT: M^-1 S M restricted to the even subspace (rest + direction pairs), lbm_hot.cuh
+    CT mrt_co[2][9][9];    //      ... and to the odd subspace (pair differences)
+    CT c_feq_a[2], c_feq_b[2], c_keep[2];  // f* = c_keep f + c_feq_a feq(u_a) + c_feq_b feq(u + du)  (BGK; lbm_hot.cuh)
     CT wref[19];       // w_i * rho_ref
     int psi_kind[2];
     CT eos_a[2], eos_b[2], eos_RT[2], eos_aalpha[2], eos_sqrtT[2], eos_alpha[2], eos_rho0[2], eos_inv_gkk2[2];
@@ -226,21 +227,18 @@ __device__ __forceinline__ int nbr_offset(const Cell& c) {
 template <class L, class CT, class ST, bool BND>
 __device__ __forceinline__ void pull(const KParams<CT>& p, const Cell& c, uint32_t fl, int k, CT (&f)[L::Q]) {
     const ST* base = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.plane;
-    const bool local = p.local != 0;
     static_for<0, L::Q>([&](auto I) {
         constexpr int i = I;
         constexpr int ex = L::E[i][0], ey = L::E[i][1], ez = L::E[i][2];
         constexpr int ib = opposite<L>(i);
         const ST* src = base + (long long)i * p.plane + c.id;
-        if (!local) {
-            if constexpr (i > 0) {
-                int off = nbr_offset<-ex, -ey, -ez>(c);
-                if constexpr (BND) {
-                    if ((fl >> i) & 1u) src = base + (long long)ib * p.plane + c.id;
-                    else src += off;
-                } else {
-                    src += off;
-                }
+        if constexpr (i > 0) {
+            int off = nbr_offset<-ex, -ey, -ez>(c);
+            if constexpr (BND) {
+                if ((fl >> i) & 1u) src = base + (long long)ib * p.plane + c.id;
+                else src += off;
+            } else {
+                src += off;
             }
         }
         f[i] = Conv<CT, ST>::ld(src) + p.wref[i];
@@ -287,28 +285,6 @@ __device__ __forceinline__ CT feq(CT r, const CT (&u)[3], CT uu15) {
     if constexpr (ez == 1) eu += u[2];
     if constexpr (ez == -1) eu -= u[2];
     return w * r * (CT(1) + CT(3) * eu + CT(4.5) * eu * eu - uu15);
-}
-
-// ------------------------------------------------------------------ K1: moments + psi
-template <class L, int NC, class CT, class ST, bool BND>
-__global__ void __launch_bounds__(256) k_moments(const __grid_constant__ KParams<CT> p) {
-    const int id = blockIdx.x * blockDim.x + threadIdx.x;
-    if (id >= p.N) return;
-    uint32_t fl = 0;
-    if constexpr (BND) {
-        fl = __ldg(p.flags + id);
-        if (fl & SOLID_BIT) return;
-    }
-    const Cell c = make_cell<L>(p, id);
-#pragma unroll
-    for (int k = 0; k < NC; ++k) {
-        CT f[L::Q];
-        pull<L, CT, ST, BND>(p, c, fl, k, f);
-        CT r = CT(0);
-        static_for<0, L::Q>([&](auto I) { r += f[I]; });
-        p.psi[(long long)k * p.N + id] = psi_of_rho(p, k, r);
-        if (p.write_rho) p.rho[(long long)k * p.N + id] = r;
-    }
 }
 
 // ------------------------------------------------------------------ K1b: virtual density at boundary solids
@@ -389,156 +365,6 @@ __device__ __forceinline__ int crossed_face(const KParams<CT>& p, const Cell& c)
     return -1;
 }
 
-// ------------------------------------------------------------------ K2: fused stream + force + collide + boundary
-template <class L, int NC, class CT, class ST, int COLL, bool BND>
-__global__ void __launch_bounds__(128) k_step(const __grid_constant__ KParams<CT> p) {
-    const int id = blockIdx.x * blockDim.x + threadIdx.x;
-    if (id >= p.N) return;
-    uint32_t fl = 0;
-    if constexpr (BND) {
-        fl = __ldg(p.flags + id);
-        if (fl & SOLID_BIT) return;
-    }
-    const Cell c = make_cell<L>(p, id);
-
-    // S7 (read side) + S1: pull, moments in index order
-    CT f[NC][L::Q], rho[NC], j[NC][3];
-#pragma unroll
-    for (int k = 0; k < NC; ++k) {
-        pull<L, CT, ST, BND>(p, c, fl, k, f[k]);
-        CT r = CT(0), jx = CT(0), jy = CT(0), jz = CT(0);
-        static_for<0, L::Q>([&](auto I) {
-            constexpr int i = I;
-            const CT v = f[k][i];
-            r += v;
-            if constexpr (L::E[i][0] == 1) jx += v;
-            if constexpr (L::E[i][0] == -1) jx -= v;
-            if constexpr (L::E[i][1] == 1) jy += v;
-            if constexpr (L::E[i][1] == -1) jy -= v;
-            if constexpr (L::E[i][2] == 1) jz += v;
-            if constexpr (L::E[i][2] == -1) jz -= v;
-        });
-        rho[k] = r; j[k][0] = jx; j[k][1] = jy; j[k][2] = jz;
-    }
-
-    CT u[3] = {CT(0), CT(0), CT(0)};
-    CT du[NC][3];
-    if (!p.no_collide) {
-        // S4: interaction force F^k = -psi^k(x) sum_k' g_kk' S^k'
-        CT S[NC][3];
-        psi_gradient_sums<L, NC, CT>(p, c, S);
-#pragma unroll
-        for (int k = 0; k < NC; ++k) {
-            const CT mpsi = -__ldg(p.psi + (long long)k * p.N + id);
-            const CT inv_r = CT(1) / rho[k];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                CT acc = CT(0);
-#pragma unroll
-                for (int kp = 0; kp < NC; ++kp) acc += p.G[k][kp] * S[kp][a];
-                du[k][a] = (mpsi * acc) * inv_r;  // Eq. 5: Delta u = F / rho
-            }
-        }
-        // S5: common velocity (R6)
-        if constexpr (NC == 1) {
-            const CT inv_r = CT(1) / rho[0];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) u[a] = j[0][a] * inv_r;
-        } else {
-            CT den = CT(0);
-#pragma unroll
-            for (int k = 0; k < NC; ++k) den += rho[k] * p.inv_tau[k];
-            const CT inv_den = CT(1) / den;
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                CT num = CT(0);
-#pragma unroll
-                for (int k = 0; k < NC; ++k) num += j[k][a] * p.inv_tau[k];
-                u[a] = num * inv_den;
-            }
-        }
-    }
-    const CT uu15_bare = CT(1.5) * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
-
-    // S6 + S7 (write side) per component
-#pragma unroll
-    for (int k = 0; k < NC; ++k) {
-        CT fs[L::Q];
-        if (p.no_collide) {
-            static_for<0, L::Q>([&](auto I) { fs[I] = f[k][I]; });
-        } else {
-            const CT r = rho[k];
-            CT ueq[3] = {u[0], u[1], u[2]};
-            if (p.forcing == 1) {  // velocity shift (R7)
-#pragma unroll
-                for (int a = 0; a < 3; ++a) ueq[a] = u[a] + p.tau[k] * du[k][a];
-            }
-            const CT uu15 = CT(1.5) * (ueq[0] * ueq[0] + ueq[1] * ueq[1] + ueq[2] * ueq[2]);
-            CT fe[L::Q];
-            static_for<0, L::Q>([&](auto I) { fe[I] = feq<L, I, CT>(r, ueq, uu15); });
-            if constexpr (COLL == 0) {
-                const CT om = p.inv_tau[k];
-                static_for<0, L::Q>([&](auto I) { fs[I] = f[k][I] - om * (f[k][I] - fe[I]); });
-            } else {
-                // MRT: f* = f - M^-1 S M (f - f_eq); M^-1 = M^T diag(1/|row|^2)
-                CT neq[L::Q];
-                static_for<0, L::Q>([&](auto I) { neq[I] = f[k][I] - fe[I]; fs[I] = f[k][I]; });
-                static_for<0, L::Q>([&](auto R) {
-                    constexpr int r_ = R;
-                    CT m = CT(0);
-                    static_for<0, L::Q>([&](auto I) {
-                        constexpr int e2 = mrt_entry2<L>(r_, I);
-                        if constexpr (e2 != 0) m += CT(0.5 * e2) * neq[I];
-                    });
-                    m *= p.mrt_s[k][r_] * (CT(1) / CT(mrt_norm2<L>(r_) ));
-                    static_for<0, L::Q>([&](auto I) {
-                        constexpr int e2 = mrt_entry2<L>(r_, I);
-                        if constexpr (e2 != 0) fs[I] -= CT(0.5 * e2) * m;
-                    });
-                });
-            }
-            if (p.forcing == 0) {  // EDM (Eq. 5): f* += f_eq(rho, u+du) - f_eq(rho, u)
-                const CT up[3] = {u[0] + du[k][0], u[1] + du[k][1], u[2] + du[k][2]};
-                const CT uu15p = CT(1.5) * (up[0] * up[0] + up[1] * up[1] + up[2] * up[2]);
-                static_for<0, L::Q>([&](auto I) { fs[I] += feq<L, I, CT>(r, up, uu15p) - fe[I]; });
-            }
-        }
-        // boundary rules applied at the writing cell for links across velocity / pressure faces (R10)
-        if constexpr (BND) {
-            if (fl & FACEBC_BIT) {
-                static_for<1, L::Q>([&](auto O) {
-                    constexpr int o = O;
-                    constexpr int eox = L::E[o][0], eoy = L::E[o][1], eoz = L::E[o][2];
-                    constexpr CT w = CT(L::WN[o]) / CT(L::WD);
-                    const int face = crossed_face<L, o>(p, c);
-                    if (face >= 0) {
-                        const int kind = p.face_kind[face];
-                        // the arriving direction is i = opposite(o), e_i = -e_o
-                        if (kind == FACE_VELOCITY) {
-                            CT eu = CT(0);
-                            if constexpr (eox != 0) eu -= CT(eox) * p.face_u[face][0];
-                            if constexpr (eoy != 0) eu -= CT(eoy) * p.face_u[face][1];
-                            if constexpr (eoz != 0) eu -= CT(eoz) * p.face_u[face][2];
-                            fs[o] = fs[o] + CT(2) * w * p.face_rho[face][k] * eu * CT(3);
-                        } else if (kind == FACE_PRESSURE) {
-                            CT eu = CT(0);
-                            if constexpr (eox != 0) eu += CT(eox) * u[0];
-                            if constexpr (eoy != 0) eu += CT(eoy) * u[1];
-                            if constexpr (eoz != 0) eu += CT(eoz) * u[2];
-                            fs[o] = -fs[o] + CT(2) * w * p.face_rho[face][k] * (CT(1) + CT(4.5) * eu * eu - uu15_bare);
-                        }
-                    }
-                });
-            }
-        }
-        ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.plane + id;
-        static_for<0, L::Q>([&](auto I) {
-            constexpr int i = I;
-            Conv<CT, ST>::st(out + (long long)i * p.plane, fs[i] - p.wref[i]);
-        });
-    }
-}
-
 // ------------------------------------------------------------------ S0: initialisation
 // io.in[k] = rho^k, io.in[2+a] = u_a (NULL = 0) for cells [c0, c0+cnt)
 template <class L, int NC, class CT, class ST>
@@ -565,7 +391,39 @@ __global__ void __launch_bounds__(256) k_init(const __grid_constant__ KParams<CT
             constexpr int i = I;
             const CT v = feq<L, i, CT>(r, u, uu15) - p.wref[i];
             Conv<CT, ST>::st(a_ + (long long)i * p.plane, v);
-            if (solid) Conv<CT, ST>::st(b_ + (long long)i * p.plane, v);
+            Conv<CT, ST>::st(b_ + (long long)i * p.plane, v);
+        });
+    }
+}
+
+// Post-stream f(x,0) in f_in  ->  storage convention in f_out (see the header of this file): a pure scatter of
+// stored values (no arithmetic), race-free because every slot has at most one writer; slots nobody writes keep
+// the copy k_init / k_import_pop left there.
+template <class L, int NC, class ST, class CT, bool BND>
+__global__ void __launch_bounds__(256) k_unstream(const __grid_constant__ KParams<CT> p, int only_k /* -1 = all */) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= p.N) return;
+    uint32_t fl = 0;
+    if constexpr (BND) {
+        fl = __ldg(p.flags + id);
+        if (fl & SOLID_BIT) return;
+    }
+    const Cell c = make_cell<L>(p, id);
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        if (only_k >= 0 && k != only_k) continue;
+        const ST* in = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.plane + id;
+        ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.plane + id;
+        static_for<0, L::Q>([&](auto I) {
+            constexpr int i = I;
+            constexpr int ib = opposite<L>(i);
+            const ST v = in[(long long)i * p.plane];
+            if constexpr (i == 0) {
+                out[0] = v;
+            } else {
+                if (BND && ((fl >> i) & 1u)) out[(long long)ib * p.plane] = v;
+                else out[(long long)i * p.plane + nbr_offset<-L::E[i][0], -L::E[i][1], -L::E[i][2]>(c)] = v;
+            }
         });
     }
 }

@@ -1,0 +1,512 @@
+// lbm_hot.cuh -- the hot-loop kernels of the Shan-Chen LBM step for sm_100a.
+//
+//   k_moments_v  K1   S1 (rho) + S3 (psi)                      Eq. 4/10, Eq. 12
+//   k_step_v     K2   S1 (j) + S4..S7 fused                     Eq. 13, Eq. 3, Eq. 5,
+//                                                               Eq. 2, bounce-back P:219, faces P:313
+//
+// Design for B200 (the step is an HBM-bound stencil; the first one-thread-per-cell version was issue-bound at
+// ~930 instructions per cell, profiles/r01_*):
+//   * every thread owns VEC consecutive cells of one x-row; the population planes are read and written with
+//     128-bit (or 64-bit) vector accesses.  Stores are always aligned because the planes hold post-collision
+//     values at the cell that computed them; a pull along +-x is the aligned vector of the row plus ONE scalar
+//     from the neighbouring vector (an L1 hit);
+//   * index arithmetic (two integer divisions, wrap/clamp of the 3x3 row neighbourhood) is paid once per thread;
+//   * the arithmetic is organised over the (i, ibar) direction pairs: sums and differences give the moments,
+//     the two equilibria of a pair share their even part, and MRT is applied as two small dense blocks
+//     (even / odd subspace of M^-1 S M, precomputed on the host) instead of two 19x19 products.
+// Summation order therefore differs from the oracle's index order: parity holds to rounding.
+#pragma once
+#include "lbm_core.cuh"
+
+namespace lbmk {
+
+// ------------------------------------------------------------------ vector load / store in the storage dtype
+template <int BYTES> struct RawVec;
+template <> struct RawVec<2> { using type = unsigned short; };
+template <> struct RawVec<4> { using type = unsigned int; };
+template <> struct RawVec<8> { using type = uint2; };
+template <> struct RawVec<16> { using type = uint4; };
+
+template <class CT, class ST> struct Cvt;
+template <> struct Cvt<float, float> {
+    static __device__ __forceinline__ float up(float v) { return v; }
+    static __device__ __forceinline__ float down(float v) { return v; }
+};
+template <> struct Cvt<double, double> {
+    static __device__ __forceinline__ double up(double v) { return v; }
+    static __device__ __forceinline__ double down(double v) { return v; }
+};
+template <> struct Cvt<float, __half> {
+    static __device__ __forceinline__ float up(__half v) { return __half2float(v); }
+    static __device__ __forceinline__ __half down(float v) { return __float2half_rn(v); }  // R16: RNE once, at the store
+};
+template <> struct Cvt<double, float> {
+    static __device__ __forceinline__ double up(float v) { return (double)v; }
+    static __device__ __forceinline__ float down(double v) { return __double2float_rn(v); }
+};
+
+template <> struct Cvt<uint32_t, uint32_t> {
+    static __device__ __forceinline__ uint32_t up(uint32_t v) { return v; }
+    static __device__ __forceinline__ uint32_t down(uint32_t v) { return v; }
+};
+
+template <class CT, class ST, int VEC>
+__device__ __forceinline__ void ld_vec(const ST* __restrict__ p, CT (&out)[VEC]) {
+    using R = typename RawVec<sizeof(ST) * VEC>::type;
+    const R r = __ldg(reinterpret_cast<const R*>(p));
+    const ST* t = reinterpret_cast<const ST*>(&r);
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) out[v] = Cvt<CT, ST>::up(t[v]);
+}
+template <class CT, class ST>
+__device__ __forceinline__ CT ld_one(const ST* __restrict__ p) {
+    CT t[1];
+    ld_vec<CT, ST, 1>(p, t);
+    return t[0];
+}
+template <class CT, class ST, int VEC>
+__device__ __forceinline__ void st_vec(ST* __restrict__ p, const CT (&in)[VEC]) {
+    using R = typename RawVec<sizeof(ST) * VEC>::type;
+    R r;
+    ST* t = reinterpret_cast<ST*>(&r);
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) t[v] = Cvt<CT, ST>::down(in[v]);
+    *reinterpret_cast<R*>(p) = r;
+}
+
+// ------------------------------------------------------------------ geometry of a thread's VEC cells
+struct VCell {
+    int id0;       // cell index of lane 0
+    int x0, y, z;
+    int xm, xp;    // x index left of lane 0 / right of lane VEC-1 (wrap, or clamp on a non-periodic axis: R10)
+    int yo[3];     // element offset of rows y-1, y, y+1 (wrap / clamp)
+    int zo[3];     // element offset of planes z-1, z, z+1
+};
+
+template <class L, int VEC, class CT>
+__device__ __forceinline__ VCell make_vcell(const KParams<CT>& p, unsigned vid) {
+    VCell c;
+    const unsigned nxv = (unsigned)p.nx / VEC;
+    const unsigned r = vid / nxv;
+    c.x0 = (int)(vid - r * nxv) * VEC;
+    if constexpr (L::D == 3) {
+        c.z = (int)(r / (unsigned)p.ny);
+        c.y = (int)(r - (unsigned)c.z * (unsigned)p.ny);
+    } else {
+        c.z = 0;
+        c.y = (int)r;
+    }
+    const int sy = p.nx, sz = p.nx * p.ny;
+    c.xm = c.x0 > 0 ? c.x0 - 1 : (p.periodic[0] ? p.nx - 1 : 0);
+    c.xp = c.x0 + VEC < p.nx ? c.x0 + VEC : (p.periodic[0] ? 0 : p.nx - 1);
+    c.yo[1] = c.y * sy;
+    c.yo[0] = c.y > 0 ? c.yo[1] - sy : (p.periodic[1] ? (p.ny - 1) * sy : c.yo[1]);
+    c.yo[2] = c.y < p.ny - 1 ? c.yo[1] + sy : (p.periodic[1] ? 0 : c.yo[1]);
+    if constexpr (L::D == 3) {
+        c.zo[1] = c.z * sz;
+        c.zo[0] = c.z > 0 ? c.zo[1] - sz : (p.periodic[2] ? (p.nz - 1) * sz : c.zo[1]);
+        c.zo[2] = c.z < p.nz - 1 ? c.zo[1] + sz : (p.periodic[2] ? 0 : c.zo[1]);
+    } else {
+        c.zo[0] = c.zo[1] = c.zo[2] = 0;
+    }
+    c.id0 = c.zo[1] + c.yo[1] + c.x0;
+    return c;
+}
+
+// S7 read side for VEC cells: f[i][v] = stored_i(x_v - e_i), or stored_ibar(x_v) on a flagged link.
+template <class L, class CT, class ST, bool BND, int VEC>
+__device__ __forceinline__ void pull_vec(const KParams<CT>& p, const VCell& c, const uint32_t (&fl)[VEC], int k,
+                                         CT (&f)[L::Q][VEC]) {
+    const ST* base = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.plane;
+    uint32_t any = 0;
+    if constexpr (BND) {
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) any |= fl[v];
+    }
+    static_for<0, L::Q>([&](auto I) {
+        constexpr int i = I;
+        constexpr int ex = L::E[i][0], ey = L::E[i][1], ez = L::E[i][2];
+        const ST* row = base + (long long)i * p.plane + (c.zo[1 - ez] + c.yo[1 - ey]);
+        if constexpr (ex == 0) {
+            ld_vec<CT, ST, VEC>(row + c.x0, f[i]);
+        } else if constexpr (VEC == 1) {
+            f[i][0] = ld_one<CT, ST>(row + (ex > 0 ? c.xm : c.xp));
+        } else {
+            CT t[VEC];
+            ld_vec<CT, ST, VEC>(row + c.x0, t);
+            if constexpr (ex > 0) {
+                f[i][0] = ld_one<CT, ST>(row + c.xm);
+#pragma unroll
+                for (int v = 1; v < VEC; ++v) f[i][v] = t[v - 1];
+            } else {
+#pragma unroll
+                for (int v = 0; v < VEC - 1; ++v) f[i][v] = t[v + 1];
+                f[i][VEC - 1] = ld_one<CT, ST>(row + c.xp);
+            }
+        }
+        if constexpr (BND && i > 0) {
+            if ((any >> i) & 1u) {
+                constexpr int ib = opposite<L>(i);
+                CT own[VEC];
+                ld_vec<CT, ST, VEC>(base + (long long)ib * p.plane + c.id0, own);
+#pragma unroll
+                for (int v = 0; v < VEC; ++v)
+                    if ((fl[v] >> i) & 1u) f[i][v] = own[v];
+            }
+        }
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) f[i][v] += p.wref[i];
+    });
+}
+
+// link flags of the thread's cells; returns false when every lane is solid (nothing to do)
+template <bool BND, int VEC, class CT>
+__device__ __forceinline__ bool load_flags(const KParams<CT>& p, const VCell& c, uint32_t (&fl)[VEC]) {
+    if constexpr (!BND) {
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) fl[v] = 0;
+        return true;
+    } else {
+        ld_vec<uint32_t, uint32_t, VEC>(p.flags + c.id0, fl);
+        uint32_t all = SOLID_BIT;
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) all &= fl[v];
+        return all == 0;
+    }
+}
+
+// store VEC values of one field; solid lanes are skipped
+template <class CT, class ST, bool BND, int VEC>
+__device__ __forceinline__ void store_lanes(ST* __restrict__ dst, const CT (&val)[VEC], const uint32_t (&fl)[VEC]) {
+    if constexpr (BND) {
+        uint32_t anys = 0;
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) anys |= fl[v];
+        if (anys & SOLID_BIT) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v)
+                if (!(fl[v] & SOLID_BIT)) dst[v] = Cvt<CT, ST>::down(val[v]);
+            return;
+        }
+    }
+    st_vec<CT, ST, VEC>(dst, val);
+}
+
+// ------------------------------------------------------------------ arithmetic over direction pairs
+// Both lattices list direction 2p+1 and its opposite 2p+2 next to each other (include/lbm.h).
+template <class L>
+constexpr bool pairs_ok() {
+    for (int pq = 0; pq < (L::Q - 1) / 2; ++pq)
+        if (opposite<L>(2 * pq + 1) != 2 * pq + 2) return false;
+    return true;
+}
+static_assert(pairs_ok<D2Q9>() && pairs_ok<D3Q19>(), "direction order must list opposite pairs");
+
+// S1: rho = sum f, j = sum f e  (Eq. 4, 10)
+template <class L, class CT>
+__device__ __forceinline__ void moments(const CT (&f)[L::Q], CT& rho, CT (&j)[3]) {
+    CT r = f[0], jx = CT(0), jy = CT(0), jz = CT(0);
+    static_for<0, (L::Q - 1) / 2>([&](auto P) {
+        constexpr int a = 2 * P + 1, b = a + 1;
+        const CT s = f[a] + f[b], d = f[a] - f[b];
+        r += s;
+        if constexpr (L::E[a][0] == 1) jx += d;
+        if constexpr (L::E[a][0] == -1) jx -= d;
+        if constexpr (L::E[a][1] == 1) jy += d;
+        if constexpr (L::E[a][1] == -1) jy -= d;
+        if constexpr (L::E[a][2] == 1) jz += d;
+        if constexpr (L::E[a][2] == -1) jz -= d;
+    });
+    rho = r; j[0] = jx; j[1] = jy; j[2] = jz;
+}
+template <class L, class CT>
+__device__ __forceinline__ CT density(const CT (&f)[L::Q]) {
+    CT r = f[0];
+    static_for<0, (L::Q - 1) / 2>([&](auto P) { r += f[2 * P + 1] + f[2 * P + 2]; });
+    return r;
+}
+
+// acc_i += coef * f_eq,i(rho, u)   (R1: f_eq = w rho [1 + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u]); a pair shares its even part
+template <class L, class CT>
+__device__ __forceinline__ void add_feq(CT coef, CT rho, const CT (&u)[3], CT (&acc)[L::Q]) {
+    const CT cr = coef * rho;
+    const CT c0 = CT(1) - CT(1.5) * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+    acc[0] += (cr * (CT(L::WN[0]) / CT(L::WD))) * c0;
+    static_for<0, (L::Q - 1) / 2>([&](auto P) {
+        constexpr int a = 2 * P + 1, b = a + 1;
+        constexpr int ex = L::E[a][0], ey = L::E[a][1], ez = L::E[a][2];
+        CT eu = CT(0);
+        if constexpr (ex == 1) eu += u[0];
+        if constexpr (ex == -1) eu -= u[0];
+        if constexpr (ey == 1) eu += u[1];
+        if constexpr (ey == -1) eu -= u[1];
+        if constexpr (ez == 1) eu += u[2];
+        if constexpr (ez == -1) eu -= u[2];
+        const CT wr = cr * (CT(L::WN[a]) / CT(L::WD));
+        const CT even = c0 + CT(4.5) * eu * eu;
+        const CT odd = CT(3) * eu;
+        acc[a] += wr * (even + odd);
+        acc[b] += wr * (even - odd);
+    });
+}
+
+// S6 for one cell and one component.  u: common velocity u' (R6); du = F/rho (Eq. 5).
+//   BGK : f* = c_keep f + c_feq_a f_eq(u_a) + c_feq_b f_eq(u' + du)
+//         EDM   (Eq. 3 + Eq. 5): u_a = u', c_keep = 1 - 1/tau, c_feq_a = 1/tau - 1, c_feq_b = 1
+//         SHIFT (R7)           : u_a = u' + tau du, c_keep = 1 - 1/tau, c_feq_a = 1/tau, c_feq_b = 0
+//   MRT : f* = f - M^-1 S M (f - f_eq(u_a)) [+ f_eq(u' + du) - f_eq(u') for EDM], with M^-1 S M applied as its
+//         even block (on f_0 and the pair sums) and odd block (on the pair differences): rows of M are even or
+//         odd polynomials of c (R9), so M^-1 S M = C_even + C_odd with no cross terms.
+template <class L, int COLL, class CT>
+__device__ __forceinline__ void collide(const KParams<CT>& p, int k, CT rho, const CT (&u)[3], const CT (&du)[3],
+                                        CT (&f)[L::Q]) {
+    constexpr int NP = (L::Q - 1) / 2;
+    const bool shift = p.forcing == 1;
+    CT ua[3], ub[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        ub[a] = u[a] + du[a];
+        ua[a] = shift ? u[a] + p.tau[k] * du[a] : u[a];
+    }
+    if constexpr (COLL == 0) {
+        const CT keep = p.c_keep[k], ca = p.c_feq_a[k], cb = p.c_feq_b[k];
+        static_for<0, L::Q>([&](auto I) { f[I] *= keep; });
+        if (ca != CT(0)) add_feq<L, CT>(ca, rho, ua, f);
+        if (cb != CT(0)) add_feq<L, CT>(cb, rho, ub, f);
+    } else {
+        CT e[L::Q];
+        static_for<0, L::Q>([&](auto I) { e[I] = CT(0); });
+        add_feq<L, CT>(CT(1), rho, ua, e);
+        CT sn[NP + 1], dn[NP];
+        sn[0] = f[0] - e[0];
+        static_for<0, NP>([&](auto P) {
+            constexpr int a = 2 * P + 1, b = a + 1;
+            const CT na = f[a] - e[a], nb = f[b] - e[b];
+            sn[P + 1] = na + nb;
+            dn[P] = na - nb;
+        });
+        static_for<0, NP + 1>([&](auto R) {
+            CT re = CT(0);
+            static_for<0, NP + 1>([&](auto C_) { re += p.mrt_ce[k][R][C_] * sn[C_]; });
+            if constexpr (R == 0) {
+                f[0] -= re;
+            } else {
+                CT ro = CT(0);
+                static_for<0, NP>([&](auto C_) { ro += p.mrt_co[k][R - 1][C_] * dn[C_]; });
+                f[2 * R - 1] -= re + ro;
+                f[2 * R] -= re - ro;
+            }
+        });
+        if (!shift) {  // EDM source (Eq. 5)
+            static_for<0, L::Q>([&](auto I) { f[I] -= e[I]; });
+            add_feq<L, CT>(CT(1), rho, ub, f);
+        }
+    }
+}
+
+// which (dy,dz) rows of the 3x3 neighbourhood does the lattice touch, and with which dx
+template <class L>
+constexpr bool row_has(int dy, int dz, int dx) {
+    for (int i = 1; i < L::Q; ++i)
+        if (L::E[i][0] == dx && L::E[i][1] == dy && L::E[i][2] == dz) return true;
+    return false;
+}
+template <class L>
+constexpr int dir_of(int dx, int dy, int dz) {
+    for (int i = 0; i < L::Q; ++i)
+        if (L::E[i][0] == dx && L::E[i][1] == dy && L::E[i][2] == dz) return i;
+    return -1;
+}
+
+// S4 sums for VEC cells: S[a][v] = sum_i (w_i/cs2) psi(x_v + e_i) e_ia  and psi at the cells themselves
+template <class L, class CT, int VEC>
+__device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VCell& c, CT (&S)[3][VEC], CT (&pc)[VEC]) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) S[a][v] = CT(0);
+    static_for<0, 9>([&](auto RW) {
+        constexpr int dy = RW % 3 - 1, dz = RW / 3 - 1;
+        constexpr bool centre = dy == 0 && dz == 0;
+        constexpr bool has0 = row_has<L>(dy, dz, 0), hasx = row_has<L>(dy, dz, 1);
+        if constexpr ((has0 || hasx || centre) && (L::D == 3 || dz == 0)) {
+            const CT* row = ps + (c.zo[1 + dz] + c.yo[1 + dy]);
+            CT t[VEC];
+            ld_vec<CT, CT, VEC>(row + c.x0, t);
+            if constexpr (centre) {
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) pc[v] = t[v];
+            }
+            if constexpr (has0) {
+                constexpr int i = dir_of<L>(0, dy, dz);
+                constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) {
+                    if constexpr (dy != 0) S[1][v] += CT(gw * dy) * t[v];
+                    if constexpr (dz != 0) S[2][v] += CT(gw * dz) * t[v];
+                }
+            }
+            if constexpr (hasx) {
+                constexpr int i = dir_of<L>(1, dy, dz);
+                constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
+                const CT left = __ldg(row + c.xm), right = __ldg(row + c.xp);
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) {
+                    const CT m = v > 0 ? t[v - 1] : left;
+                    const CT q = v < VEC - 1 ? t[v + 1] : right;
+                    S[0][v] += gw * (q - m);
+                    if constexpr (dy != 0) S[1][v] += CT(gw * dy) * (q + m);
+                    if constexpr (dz != 0) S[2][v] += CT(gw * dz) * (q + m);
+                }
+            }
+        }
+    });
+}
+
+// ------------------------------------------------------------------ K1: rho + psi
+template <class L, int NC, class CT, class ST, bool BND, int VEC>
+__global__ void __launch_bounds__(256) k_moments_v(const __grid_constant__ KParams<CT> p) {
+    const unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (vid >= (unsigned)p.N / VEC) return;
+    const VCell c = make_vcell<L, VEC>(p, vid);
+    uint32_t fl[VEC];
+    if (!load_flags<BND, VEC>(p, c, fl)) return;
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        CT f[L::Q][VEC];
+        pull_vec<L, CT, ST, BND, VEC>(p, c, fl, k, f);
+        CT r[VEC], ps[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            CT fc[L::Q];
+            static_for<0, L::Q>([&](auto I) { fc[I] = f[I][v]; });
+            r[v] = density<L, CT>(fc);
+            ps[v] = psi_of_rho(p, k, r[v]);
+        }
+        store_lanes<CT, CT, BND, VEC>(p.psi + (long long)k * p.N + c.id0, ps, fl);
+        if (p.write_rho) store_lanes<CT, CT, BND, VEC>(p.rho + (long long)k * p.N + c.id0, r, fl);
+    }
+}
+
+// ------------------------------------------------------------------ K2: fused stream + force + collide + boundary
+// COLL: 0 BGK, 1 MRT, 2 none (LBM_FLAG_NO_COLLIDE: pure streaming)
+template <class L, int NC, class CT, class ST, int COLL, bool BND, int VEC>
+__global__ void __launch_bounds__(128) k_step_v(const __grid_constant__ KParams<CT> p) {
+    const unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (vid >= (unsigned)p.N / VEC) return;
+    const VCell c = make_vcell<L, VEC>(p, vid);
+    uint32_t fl[VEC];
+    if (!load_flags<BND, VEC>(p, c, fl)) return;
+
+    // S7 (read side) + S1
+    CT f[NC][L::Q][VEC], rho[NC][VEC], j[NC][3][VEC];
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        pull_vec<L, CT, ST, BND, VEC>(p, c, fl, k, f[k]);
+        if constexpr (COLL != 2) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                CT fc[L::Q], jj[3];
+                static_for<0, L::Q>([&](auto I) { fc[I] = f[k][I][v]; });
+                moments<L, CT>(fc, rho[k][v], jj);
+                j[k][0][v] = jj[0]; j[k][1][v] = jj[1]; j[k][2][v] = jj[2];
+            }
+        }
+    }
+
+    CT u[3][VEC], du[NC][3][VEC];
+    if constexpr (COLL != 2) {
+        // S4: F^k = -psi^k(x) sum_k' g_kk' S^k'   (Eq. 13);  du = F / rho (Eq. 5)
+        CT S[NC][3][VEC], pc[NC][VEC];
+#pragma unroll
+        for (int kp = 0; kp < NC; ++kp) psi_sums_vec<L, CT, VEC>(p.psi + (long long)kp * p.N, c, S[kp], pc[kp]);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            CT inv_r[NC];
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {
+                inv_r[k] = CT(1) / rho[k][v];
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    CT acc = CT(0);
+#pragma unroll
+                    for (int kp = 0; kp < NC; ++kp) acc += p.G[k][kp] * S[kp][a][v];
+                    du[k][a][v] = (-pc[k][v] * acc) * inv_r[k];
+                }
+            }
+            // S5: common velocity (R6)
+            if constexpr (NC == 1) {
+#pragma unroll
+                for (int a = 0; a < 3; ++a) u[a][v] = j[0][a][v] * inv_r[0];
+            } else {
+                CT den = CT(0);
+#pragma unroll
+                for (int k = 0; k < NC; ++k) den += rho[k][v] * p.inv_tau[k];
+                const CT inv_den = CT(1) / den;
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    CT num = CT(0);
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) num += j[k][a][v] * p.inv_tau[k];
+                    u[a][v] = num * inv_den;
+                }
+            }
+        }
+    } else {
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) u[a][v] = CT(0);
+    }
+
+    // S6 + S7 (write side)
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            if (BND && (fl[v] & SOLID_BIT)) continue;
+            CT fc[L::Q];
+            static_for<0, L::Q>([&](auto I) { fc[I] = f[k][I][v]; });
+            const CT uc[3] = {u[0][v], u[1][v], u[2][v]};
+            if constexpr (COLL != 2) {
+                const CT dc[3] = {du[k][0][v], du[k][1][v], du[k][2][v]};
+                collide<L, COLL, CT>(p, k, rho[k][v], uc, dc, fc);
+            }
+            // links across velocity / pressure faces: the rule is applied at the writing cell (R10)
+            if constexpr (BND) {
+                if (fl[v] & FACEBC_BIT) {
+                    Cell cc;
+                    cc.x = c.x0 + v; cc.y = c.y; cc.z = c.z;
+                    const CT uu15 = CT(1.5) * (uc[0] * uc[0] + uc[1] * uc[1] + uc[2] * uc[2]);
+                    static_for<1, L::Q>([&](auto O) {
+                        constexpr int o = O;
+                        constexpr int eox = L::E[o][0], eoy = L::E[o][1], eoz = L::E[o][2];
+                        constexpr CT w = CT(L::WN[o]) / CT(L::WD);
+                        const int face = crossed_face<L, o>(p, cc);
+                        if (face >= 0) {
+                            const int kind = p.face_kind[face];
+                            if (kind == FACE_VELOCITY) {   // arriving direction i = opposite(o), e_i = -e_o
+                                CT eu = CT(0);
+                                if constexpr (eox != 0) eu -= CT(eox) * p.face_u[face][0];
+                                if constexpr (eoy != 0) eu -= CT(eoy) * p.face_u[face][1];
+                                if constexpr (eoz != 0) eu -= CT(eoz) * p.face_u[face][2];
+                                fc[o] = fc[o] + CT(2) * w * p.face_rho[face][k] * eu * CT(3);
+                            } else if (kind == FACE_PRESSURE) {
+                                CT eu = CT(0);
+                                if constexpr (eox != 0) eu += CT(eox) * uc[0];
+                                if constexpr (eoy != 0) eu += CT(eoy) * uc[1];
+                                if constexpr (eoz != 0) eu += CT(eoz) * uc[2];
+                                fc[o] = -fc[o] + CT(2) * w * p.face_rho[face][k] * (CT(1) + CT(4.5) * eu * eu - uu15);
+                            }
+                        }
+                    });
+                }
+            }
+            static_for<0, L::Q>([&](auto I) { f[k][I][v] = fc[I] - p.wref[I]; });
+        }
+        ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.plane + c.id0;
+        static_for<0, L::Q>([&](auto I) { store_lanes<CT, ST, BND, VEC>(out + (long long)I * p.plane, f[k][I], fl); });
+    }
+}
+
+}  // namespace lbmk
