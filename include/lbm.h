@@ -86,6 +86,11 @@ enum lbm_face_kind { LBM_FACE_PERIODIC = 0, LBM_FACE_WALL = 1, LBM_FACE_VELOCITY
 
 /* flags */
 #define LBM_FLAG_NO_COLLIDE 1u /* f* = f: pure streaming, for the bit-exact permutation test */
+#define LBM_FLAG_TWO_PASS 2u   /* always run the two-pass path K1 (+K1b) + K2 */
+#define LBM_FLAG_ONE_PASS 4u   /* require the one-pass kernel K2F: lbm_step fails with LBM_E_UNSUPPORTED where it does not
+                                  apply (solid cells, a non-periodic axis, nx not a multiple of the vector width, or a
+                                  dtype/component combination it is not built for).  Default (neither flag): K2F where it
+                                  applies and the domain is large enough to fill the GPU, else two-pass. */
 
 typedef struct {
     int32_t psi_kind; /* lbm_psi_kind */

@@ -27,6 +27,8 @@ DTYPES = {"f16": 0, "f32": 1, "f64": 2}
 FACE_KINDS = {"PERIODIC": 0, "WALL": 1, "VELOCITY": 2, "PRESSURE": 3}
 KERNEL_IDS = {"moments": 0, "virtual": 1, "step": 2, "fused": 3}
 FLAG_NO_COLLIDE = 1
+FLAG_TWO_PASS = 2
+FLAG_ONE_PASS = 4
 STATUS = {0: "LBM_OK", -1: "LBM_E_INVALID", -2: "LBM_E_UNSUPPORTED", -3: "LBM_E_NOMEM", -4: "LBM_E_CUDA",
           -5: "LBM_E_STATE"}
 
@@ -121,6 +123,7 @@ def make_config(wl: dict) -> lbm_config_t:
     c.compute_dtype = DTYPES[wl.get("compute_dtype", "f64")]
     c.store_dtype = DTYPES[wl.get("store_dtype", wl.get("compute_dtype", "f64"))]
     c.flags = FLAG_NO_COLLIDE if wl.get("no_collide", False) else 0
+    c.flags |= {None: 0, "two_pass": FLAG_TWO_PASS, "one_pass": FLAG_ONE_PASS}[wl.get("path")]
     c.rho_ref = float(wl.get("rho_ref", 0.0))
     q = 9 if wl["lattice"] == "D2Q9" else 19
     G = wl.get("G", [[0.0] * nc for _ in range(nc)])

@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -23,7 +24,7 @@ size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 size_t dtype_bytes(int dt) { return dt == LBM_F16 ? 2 : dt == LBM_F32 ? 4 : 8; }
 
 struct Carve {
-    size_t f[2], psi, rho, flags, bsolid, mask, counter, stage_a, stage_b, total;
+    size_t f[2], psi, rho, flags, bsolid, flist, mask, counter, stage_a, stage_b, total;
 };
 
 }  // namespace
@@ -38,8 +39,14 @@ struct lbm {
     Carve cv;
     int cur;
     int vec;   // cells per thread in the hot kernels (1 or the dtype's vector width)
+    FusedShape fshape;   // tile of the one-pass kernel K2F (vec = 0: not built for this configuration)
+    int fvariant;        // tuning variant of K2F (0 = default)
+    int fmchunk;         // planes marched per CTA
+    bool use_fused;      // decided in prepare()
     bool initialized, has_solid, bnd, dirty, force_rho;
     int nbsolid;
+    int nfluid;       // fluid cells (masked domains)
+    bool use_list;    // hot kernels iterate over the fluid-cell list (porous domains)
     int face_kind[6];
     double face_rho[6][2], face_u[6][3];
     int64_t steps, launches;
@@ -97,6 +104,7 @@ Carve carve(const lbm_config_t& c) {
     v.rho = take(nc * N * cb);
     v.flags = take(N * 4);
     v.bsolid = take(N * 4);
+    v.flist = take(N * 4 + ((N + 1023) / 1024 + 1) * 4);   // fluid-cell list + per-block counts of its compaction
     v.mask = take(N);
     v.counter = take(256);
     const size_t chunk = std::min<size_t>(N, CHUNK_CELLS);
@@ -162,6 +170,8 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
     p.flags = reinterpret_cast<const uint32_t*>(h->ws + h->cv.flags);
     p.bsolid = reinterpret_cast<const int*>(h->ws + h->cv.bsolid);
     p.nbsolid = h->nbsolid;
+    p.flist = reinterpret_cast<const int*>(h->ws + h->cv.flist);
+    p.nfluid = h->nfluid;
     p.forcing = c.forcing == LBM_SHIFT ? 1 : 0;
     p.write_rho = (h->nbsolid > 0 || h->force_rho) ? 1 : 0;
     double w[19];
@@ -281,6 +291,48 @@ __global__ void k_list_boundary_solids(Geo g, const uint32_t* __restrict__ flags
     if (any) list[atomicAdd(counter, 1)] = id;
 }
 
+// Fluid-cell list in ascending order (stream compaction in three small kernels: per-block counts, scan, fill).
+constexpr int COMPACT_BLOCK = 1024;
+__global__ void __launch_bounds__(COMPACT_BLOCK) k_fluid_count(int N, const uint32_t* __restrict__ flags, int* __restrict__ blockcnt) {
+    const int id = blockIdx.x * COMPACT_BLOCK + threadIdx.x;
+    const int fluid = id < N && !(flags[id] & SOLID_BIT);
+    const int n = __syncthreads_count(fluid);
+    if (threadIdx.x == 0) blockcnt[blockIdx.x] = n;
+}
+// exclusive scan of nb block counts in place (one CTA); total -> blockcnt[nb]
+__global__ void __launch_bounds__(1024) k_fluid_scan(int nb, int* __restrict__ blockcnt) {
+    __shared__ int part[1024];
+    const int t = threadIdx.x;
+    const int seg = (nb + 1023) / 1024;
+    const int b0 = min(nb, t * seg), b1 = min(nb, b0 + seg);
+    int s = 0;
+    for (int b = b0; b < b1; ++b) s += blockcnt[b];
+    part[t] = s;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {
+        const int v = t >= off ? part[t - off] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    int run = part[t] - s;
+    for (int b = b0; b < b1; ++b) { const int c = blockcnt[b]; blockcnt[b] = run; run += c; }
+    if (t == 1023) blockcnt[nb] = part[1023];
+}
+__global__ void __launch_bounds__(COMPACT_BLOCK) k_fluid_fill(int N, const uint32_t* __restrict__ flags, const int* __restrict__ blockoff,
+                                                              int* __restrict__ list) {
+    __shared__ int wcnt[COMPACT_BLOCK / 32];
+    const int id = blockIdx.x * COMPACT_BLOCK + threadIdx.x;
+    const int fluid = id < N && !(flags[id] & SOLID_BIT);
+    const unsigned bal = __ballot_sync(0xffffffffu, fluid);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) wcnt[w] = __popc(bal);
+    __syncthreads();
+    int off = blockoff[blockIdx.x];
+    for (int k = 0; k < w; ++k) off += wcnt[k];
+    if (fluid) list[off + __popc(bal & ((1u << lane) - 1u))] = id;
+}
+
 __global__ void k_export_flags(int N, const uint32_t* __restrict__ in, uint32_t* __restrict__ out) {
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
     if (id < N) out[id] = in[id] & (SOLID_BIT | LINK_MASK);
@@ -351,13 +403,14 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
 
 // hot-loop launch, bracketed by events while profiling is on
 int hot_launch(lbm* h, int op, int kid) {
-    if (!h->profiling) return do_launch(h, op, nullptr, nullptr, nullptr, 0, -1, -1);
+    const int i0 = op == OP_FUSED ? h->fmchunk : 0;
+    if (!h->profiling) return do_launch(h, op, nullptr, nullptr, nullptr, i0, -1, -1);
     if (h->ev_pending.size() >= 2048) { int rc = prof_drain(h); if (rc) return rc; }
     lbm::EvPair pr;
     pr.kid = kid;
     int rc = prof_event(h, &pr.a);
     if (rc) return rc;
-    rc = do_launch(h, op, nullptr, nullptr, nullptr, 0, -1, -1);
+    rc = do_launch(h, op, nullptr, nullptr, nullptr, i0, -1, -1);
     if (rc) return rc;
     rc = prof_event(h, &pr.b);
     if (rc) return rc;
@@ -377,7 +430,9 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.coll = (h->cfg.flags & LBM_FLAG_NO_COLLIDE) ? 2 : (h->cfg.collision == LBM_MRT ? 1 : 0);
     a.bnd = h->bnd ? 1 : 0;
     a.vec = h->vec;
+    a.list = (h->use_list && (op == OP_MOMENTS || op == OP_STEP)) ? 1 : 0;
     a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
+    a.variant = h->fvariant;
     a.stream = h->stream;
     launch_fn fn = pick_launch(h->cfg);
     if (!fn) return fail(h, LBM_E_UNSUPPORTED, "dtype combination not built");
@@ -406,6 +461,47 @@ struct FieldIOAny {
 static_assert(sizeof(FieldIOAny) == sizeof(FieldIO<float>) && sizeof(FieldIOAny) == sizeof(FieldIO<double>),
               "FieldIO layout");
 
+// shape of K2F built for this configuration (mirrors the template dispatch in lbm_launch.cuh)
+FusedShape fused_shape_of(const lbm_config_t& c, int variant) {
+    FusedShape none{0, 0, 0};
+    auto pick = [&](auto L) -> FusedShape {
+        using LT = decltype(L);
+        const bool f32 = c.compute_dtype == LBM_F32;
+        if (variant > 0) {
+#ifdef LBM_FUSED_TUNING
+            if (LT::D == 3 && f32 && c.n_components == 1 && c.collision == LBM_BGK && variant <= FUSED_TUNING_VARIANTS)
+                return fused_tuning_shape(variant);
+#endif
+            return none;
+        }
+        if (f32) return c.n_components == 1 ? fused_shape<LT, float, float, 1>() : fused_shape<LT, float, float, 2>();
+        return c.n_components == 1 ? fused_shape<LT, double, double, 1>() : fused_shape<LT, double, double, 2>();
+    };
+    return c.lattice == LBM_D2Q9 ? pick(D2Q9{}) : pick(D3Q19{});
+}
+
+// Does the one-pass kernel apply, and how many planes does a CTA march?  Fully periodic, no solid cells, collision on.
+void plan_fused(lbm* h) {
+    h->use_fused = false;
+    const lbm_config_t& c = h->cfg;
+    if (c.flags & (LBM_FLAG_TWO_PASS | LBM_FLAG_NO_COLLIDE)) return;
+    if (h->bnd || h->fshape.vec == 0 || c.nx % h->fshape.vec != 0) return;
+    const int nm = h->d == 3 ? c.nz : c.ny;
+    const int tx = h->fshape.wx * 32 * h->fshape.vec;
+    const long long tiles = (long long)((c.nx + tx - 1) / tx) * (h->d == 3 ? (c.ny + h->fshape.ty - 1) / h->fshape.ty : 1);
+    // aim at ~8 waves of one CTA per SM, at least 8 planes per CTA (two extra planes are pulled per chunk)
+    int nsm = 148;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
+    long long nch = (8LL * nsm + tiles - 1) / tiles;
+    nch = std::max(1LL, std::min<long long>(nch, std::max(1, nm / 8)));
+    int mchunk = (int)((nm + nch - 1) / nch);
+    if (const char* e = std::getenv("LBM_TUNE_FUSED_MCHUNK")) mchunk = std::max(1, std::min(nm, std::atoi(e)));
+    h->fmchunk = mchunk;
+    // small domains cannot fill the GPU with marching CTAs: keep the two-pass path unless K2F is demanded
+    const long long ctas = tiles * ((nm + mchunk - 1) / mchunk);
+    h->use_fused = (c.flags & LBM_FLAG_ONE_PASS) || ctas >= 2LL * nsm;
+}
+
 Geo make_geo(const lbm* h) {
     Geo g;
     g.nx = h->cfg.nx; g.ny = h->cfg.ny; g.nz = h->cfg.nz; g.N = h->N;
@@ -419,6 +515,8 @@ int prepare(lbm* h) {
     if (!h->dirty) return LBM_OK;
     h->bnd = h->has_solid || !h->cfg.periodic[0] || !h->cfg.periodic[1] || (h->d == 3 && !h->cfg.periodic[2]);
     h->nbsolid = 0;
+    h->nfluid = h->N;
+    h->use_list = false;
     CU(cudaMemsetAsync(h->ws + h->cv.psi, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
     CU(cudaMemsetAsync(h->ws + h->cv.rho, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
     if (h->bnd) {
@@ -438,13 +536,28 @@ int prepare(lbm* h) {
             else k_list_boundary_solids<D3Q19><<<grid, block, 0, h->stream>>>(g, flags, list, counter);
             CU(cudaGetLastError());
             h->launches++;
-            int cnt = 0;
-            CU(cudaMemcpyAsync(&cnt, counter, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+            // fluid-cell list
+            const int nb = (h->N + COMPACT_BLOCK - 1) / COMPACT_BLOCK;
+            int* flist = reinterpret_cast<int*>(h->ws + h->cv.flist);
+            int* blockcnt = flist + h->N;
+            k_fluid_count<<<nb, COMPACT_BLOCK, 0, h->stream>>>(h->N, flags, blockcnt);
+            k_fluid_scan<<<1, 1024, 0, h->stream>>>(nb, blockcnt);
+            k_fluid_fill<<<nb, COMPACT_BLOCK, 0, h->stream>>>(h->N, flags, blockcnt, flist);
+            CU(cudaGetLastError());
+            h->launches += 3;
+            int cnt[2] = {0, 0};
+            CU(cudaMemcpyAsync(&cnt[0], counter, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+            CU(cudaMemcpyAsync(&cnt[1], blockcnt + nb, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
             CU(cudaStreamSynchronize(h->stream));
-            h->nbsolid = cnt;
+            h->nbsolid = cnt[0];
+            h->nfluid = cnt[1];
+            // with most cells solid the dense mapping wastes lanes and issue slots on them: one thread per fluid cell
+            h->use_list = h->nfluid < h->N / 2;
+            if (const char* e = std::getenv("LBM_TUNE_LIST")) h->use_list = std::atoi(e) != 0;
         }
     }
     h->dirty = false;
+    plan_fused(h);
     return LBM_OK;
 }
 
@@ -539,12 +652,20 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
         if (v < 1) v = 1;
         if (cfg->nx % v == 0) h->vec = v;
     }
+    h->fvariant = 0;
+    if (const char* e = std::getenv("LBM_TUNE_FUSED_VARIANT")) h->fvariant = std::atoi(e);
+    h->fshape = fused_shape_of(*cfg, h->fvariant);
+    if (h->fshape.vec == 0 && h->fvariant != 0) { h->fvariant = 0; h->fshape = fused_shape_of(*cfg, 0); }
+    h->fmchunk = 1;
+    h->use_fused = false;
     h->initialized = false;
     h->has_solid = false;
     h->dirty = true;
     h->bnd = false;
     h->force_rho = false;
     h->nbsolid = 0;
+    h->nfluid = h->N;
+    h->use_list = false;
     h->steps = 0;
     h->launches = 0;
     h->profiling = false;
@@ -653,7 +774,15 @@ int lbm_step(lbm_t* h, int n) {
     if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_step before lbm_init_fields");
     int rc = prepare(h);
     if (rc) return rc;
+    if ((h->cfg.flags & LBM_FLAG_ONE_PASS) && !h->use_fused)
+        return fail(h, LBM_E_UNSUPPORTED, "LBM_FLAG_ONE_PASS: the one-pass kernel does not apply to this configuration");
     for (int s = 0; s < n; ++s) {
+        if (h->use_fused) {
+            if ((rc = hot_launch(h, OP_FUSED, LBM_K_FUSED))) return rc;
+            h->cur ^= 1;
+            h->steps++;
+            continue;
+        }
         if (!(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) {
             if ((rc = hot_launch(h, OP_MOMENTS, LBM_K_MOMENTS))) return rc;
             if (h->nbsolid > 0 && (rc = hot_launch(h, OP_VIRTUAL, LBM_K_VIRTUAL))) return rc;

@@ -133,6 +133,8 @@ struct KParams {
     const uint32_t* flags;  // [N] (only read when BND)
     const int* bsolid; // boundary-solid list
     int nbsolid;
+    const int* flist;  // fluid-cell list, ascending (list mode of the hot kernels on porous domains)
+    int nfluid;
     // mode
     int forcing;       // 0 EDM, 1 SHIFT
     int write_rho;     // K1 also writes rho (needed by K1b and the exports)

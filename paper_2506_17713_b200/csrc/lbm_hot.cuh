@@ -318,9 +318,11 @@ constexpr int dir_of(int dx, int dy, int dz) {
     return -1;
 }
 
-// S4 sums for VEC cells: S[a][v] = sum_i (w_i/cs2) psi(x_v + e_i) e_ia  and psi at the cells themselves
-template <class L, class CT, int VEC>
-__device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VCell& c, CT (&S)[3][VEC], CT (&pc)[VEC]) {
+// S4 sums for VEC cells: S[a][v] = sum_i (w_i/cs2) psi(x_v + e_i) e_ia  and psi at the cells themselves.
+// rowfn(IC<dy>, IC<dz>, IC<need_x>, t, left, right) delivers psi of the row (y+dy, z+dz): t[v] at the thread's VEC
+// cells and, when need_x, the values left of lane 0 / right of lane VEC-1 (global memory in K2, shared memory in K2F).
+template <class L, class CT, int VEC, class RowFn>
+__device__ __forceinline__ void psi_sums_rows(RowFn&& rowfn, CT (&S)[3][VEC], CT (&pc)[VEC]) {
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -330,9 +332,8 @@ __device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VC
         constexpr bool centre = dy == 0 && dz == 0;
         constexpr bool has0 = row_has<L>(dy, dz, 0), hasx = row_has<L>(dy, dz, 1);
         if constexpr ((has0 || hasx || centre) && (L::D == 3 || dz == 0)) {
-            const CT* row = ps + (c.zo[1 + dz] + c.yo[1 + dy]);
-            CT t[VEC];
-            ld_vec<CT, CT, VEC>(row + c.x0, t);
+            CT t[VEC], left = CT(0), right = CT(0);
+            rowfn(IC<dy>{}, IC<dz>{}, IC<(hasx ? 1 : 0)>{}, t, left, right);
             if constexpr (centre) {
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) pc[v] = t[v];
@@ -349,7 +350,6 @@ __device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VC
             if constexpr (hasx) {
                 constexpr int i = dir_of<L>(1, dy, dz);
                 constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
-                const CT left = __ldg(row + c.xm), right = __ldg(row + c.xp);
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) {
                     const CT m = v > 0 ? t[v - 1] : left;
@@ -363,11 +363,65 @@ __device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VC
     });
 }
 
+// psi rows from the global psi field (two-pass path)
+template <class L, class CT, int VEC>
+__device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VCell& c, CT (&S)[3][VEC], CT (&pc)[VEC]) {
+    psi_sums_rows<L, CT, VEC>(
+        [&](auto DY, auto DZ, auto NX, CT (&t)[VEC], CT& left, CT& right) {
+            const CT* row = ps + (c.zo[1 + DZ] + c.yo[1 + DY]);
+            ld_vec<CT, CT, VEC>(row + c.x0, t);
+            if constexpr (NX != 0) { left = __ldg(row + c.xm); right = __ldg(row + c.xp); }
+        },
+        S, pc);
+}
+
+// S4 + S5 for one cell: du^k = F^k / rho^k with F^k = -psi^k sum_k' g_kk' S^k' (Eq. 13, Eq. 5) and the common
+// velocity u' (R6) from the moments.
+template <int NC, class CT>
+__device__ __forceinline__ void force_and_velocity(const KParams<CT>& p, const CT (&rho)[NC], const CT (&j)[NC][3],
+                                                   const CT (&S)[NC][3], const CT (&pc)[NC], CT (&u)[3], CT (&du)[NC][3]) {
+    CT inv_r[NC];
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        inv_r[k] = CT(1) / rho[k];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            CT acc = CT(0);
+#pragma unroll
+            for (int kp = 0; kp < NC; ++kp) acc += p.G[k][kp] * S[kp][a];
+            du[k][a] = (-pc[k] * acc) * inv_r[k];
+        }
+    }
+    if constexpr (NC == 1) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) u[a] = j[0][a] * inv_r[0];
+    } else {
+        CT den = CT(0);
+#pragma unroll
+        for (int k = 0; k < NC; ++k) den += rho[k] * p.inv_tau[k];
+        const CT inv_den = CT(1) / den;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            CT num = CT(0);
+#pragma unroll
+            for (int k = 0; k < NC; ++k) num += j[k][a] * p.inv_tau[k];
+            u[a] = num * inv_den;
+        }
+    }
+}
+
 // ------------------------------------------------------------------ K1: rho + psi
-template <class L, int NC, class CT, class ST, bool BND, int VEC>
+// LIST: thread t owns the fluid cell p.flist[t] (porous domains: the dense mapping leaves most lanes on solid cells)
+template <class L, int NC, class CT, class ST, bool BND, int VEC, bool LIST = false>
 __global__ void __launch_bounds__(256) k_moments_v(const __grid_constant__ KParams<CT> p) {
-    const unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
-    if (vid >= (unsigned)p.N / VEC) return;
+    static_assert(!LIST || (BND && VEC == 1), "list mode is one cell per thread on a masked domain");
+    unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
+    if constexpr (LIST) {
+        if (vid >= (unsigned)p.nfluid) return;
+        vid = (unsigned)__ldg(p.flist + vid);
+    } else {
+        if (vid >= (unsigned)p.N / VEC) return;
+    }
     const VCell c = make_vcell<L, VEC>(p, vid);
     uint32_t fl[VEC];
     if (!load_flags<BND, VEC>(p, c, fl)) return;
@@ -390,10 +444,16 @@ __global__ void __launch_bounds__(256) k_moments_v(const __grid_constant__ KPara
 
 // ------------------------------------------------------------------ K2: fused stream + force + collide + boundary
 // COLL: 0 BGK, 1 MRT, 2 none (LBM_FLAG_NO_COLLIDE: pure streaming)
-template <class L, int NC, class CT, class ST, int COLL, bool BND, int VEC>
+template <class L, int NC, class CT, class ST, int COLL, bool BND, int VEC, bool LIST = false>
 __global__ void __launch_bounds__(128) k_step_v(const __grid_constant__ KParams<CT> p) {
-    const unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
-    if (vid >= (unsigned)p.N / VEC) return;
+    static_assert(!LIST || (BND && VEC == 1), "list mode is one cell per thread on a masked domain");
+    unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
+    if constexpr (LIST) {
+        if (vid >= (unsigned)p.nfluid) return;
+        vid = (unsigned)__ldg(p.flist + vid);
+    } else {
+        if (vid >= (unsigned)p.N / VEC) return;
+    }
     const VCell c = make_vcell<L, VEC>(p, vid);
     uint32_t fl[VEC];
     if (!load_flags<BND, VEC>(p, c, fl)) return;
@@ -422,34 +482,20 @@ __global__ void __launch_bounds__(128) k_step_v(const __grid_constant__ KParams<
         for (int kp = 0; kp < NC; ++kp) psi_sums_vec<L, CT, VEC>(p.psi + (long long)kp * p.N, c, S[kp], pc[kp]);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
-            CT inv_r[NC];
+            CT rc[NC], jc[NC][3], Sc[NC][3], pcc[NC], uc[3], duc[NC][3];
 #pragma unroll
             for (int k = 0; k < NC; ++k) {
-                inv_r[k] = CT(1) / rho[k][v];
+                rc[k] = rho[k][v];
+                pcc[k] = pc[k][v];
 #pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    CT acc = CT(0);
-#pragma unroll
-                    for (int kp = 0; kp < NC; ++kp) acc += p.G[k][kp] * S[kp][a][v];
-                    du[k][a][v] = (-pc[k][v] * acc) * inv_r[k];
-                }
+                for (int a = 0; a < 3; ++a) { jc[k][a] = j[k][a][v]; Sc[k][a] = S[k][a][v]; }
             }
-            // S5: common velocity (R6)
-            if constexpr (NC == 1) {
+            force_and_velocity<NC, CT>(p, rc, jc, Sc, pcc, uc, duc);
 #pragma unroll
-                for (int a = 0; a < 3; ++a) u[a][v] = j[0][a][v] * inv_r[0];
-            } else {
-                CT den = CT(0);
+            for (int a = 0; a < 3; ++a) {
+                u[a][v] = uc[a];
 #pragma unroll
-                for (int k = 0; k < NC; ++k) den += rho[k][v] * p.inv_tau[k];
-                const CT inv_den = CT(1) / den;
-#pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    CT num = CT(0);
-#pragma unroll
-                    for (int k = 0; k < NC; ++k) num += j[k][a][v] * p.inv_tau[k];
-                    u[a][v] = num * inv_den;
-                }
+                for (int k = 0; k < NC; ++k) du[k][a][v] = duc[k][a];
             }
         }
     } else {

@@ -1,25 +1,51 @@
 // lbm_launch.cuh -- host-side dispatch from run-time options to the kernel templates of lbm_core.cuh.
 // One translation unit per (lattice, compute dtype, storage dtype) instantiates launch<L,CT,ST>.
 #pragma once
-#include "lbm_hot.cuh"
+#include "lbm_fused.cuh"
 
 namespace lbmk {
 
-enum Op { OP_MOMENTS = 0, OP_VIRTUAL = 1, OP_STEP = 2, OP_INIT = 3, OP_EXPORT_MACRO = 4, OP_EXPORT_POP = 5, OP_IMPORT_POP = 6, OP_UNSTREAM = 7 };
+enum Op { OP_MOMENTS = 0, OP_VIRTUAL = 1, OP_STEP = 2, OP_INIT = 3, OP_EXPORT_MACRO = 4, OP_EXPORT_POP = 5, OP_IMPORT_POP = 6, OP_UNSTREAM = 7, OP_FUSED = 8 };
 
 struct LaunchArgs {
     int op;
     int nc;    // components
     int coll;  // 0 BGK, 1 MRT, 2 none (pure streaming)
     int vec;   // cells per thread along x in the hot kernels: 1 or vec_width<CT, ST, NC>() (needs nx % vec == 0)
+    int list;  // hot kernels iterate over the fluid-cell list (one cell per thread) instead of the whole grid
     int bnd;   // any solid cell or non-periodic axis
     const void* params;  // KParams<CT>
     const void* a0;      // op-specific (FieldIO<CT>* for init / import / export_pop; u_out for export_macro)
     const void* a1;
     void* a2;
-    int i0;
+    int i0;              // op-specific integer (OP_FUSED: planes marched per CTA)
+    int variant;         // OP_FUSED: tile variant (0 = default; others are tuning experiments)
     cudaStream_t stream;
 };
+
+// Tile of the one-pass kernel K2F per (lattice, dtypes, components): VEC cells per lane, WX warps per row, TY rows.
+// VEC = 0: no one-pass kernel built for this combination (the two-pass path is used).
+struct FusedShape { int vec, wx, ty; };
+template <class L, class CT, class ST, int NC>
+constexpr FusedShape fused_shape() {
+    constexpr bool d3 = L::D == 3;
+    if (sizeof(CT) == 4) return NC == 1 ? FusedShape{4, 1, d3 ? 8 : 1} : FusedShape{2, 1, d3 ? 8 : 1};
+    return NC == 1 ? FusedShape{2, 1, d3 ? 8 : 1} : FusedShape{0, 0, 0};
+}
+// Tuning experiments of K2F (built with -DLBM_FUSED_TUNING; D3Q19, fp32 compute, one component, BGK only):
+// variant v = 1..FUSED_TUNING_VARIANTS selects {shape, L2 prefetch}; 0 is the default shape above.
+constexpr int FUSED_TUNING_VARIANTS = 6;
+constexpr FusedShape fused_tuning_shape(int v) {
+    switch (v) {
+        case 1: return {4, 1, 8};
+        case 2: return {2, 1, 14};
+        case 3: return {2, 1, 14};
+        case 4: return {2, 2, 6};
+        case 5: return {4, 1, 6};
+        default: return {2, 1, 8};
+    }
+}
+constexpr bool fused_tuning_pf(int v) { return v != 1 && v != 3; }
 
 template <class L, class CT, class ST>
 cudaError_t launch(const LaunchArgs& a);
@@ -52,6 +78,12 @@ cudaError_t launch(const LaunchArgs& a) {
             with_nc([&](auto NC) {
                 with_bnd([&](auto B) {
                     constexpr int VW = vec_width<CT, ST, NC>();
+                    if constexpr (B != 0) {
+                        if (a.list) {
+                            k_moments_v<L, NC, CT, ST, true, 1, true><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p);
+                            return;
+                        }
+                    }
                     if (a.vec == VW && VW > 1)
                         k_moments_v<L, NC, CT, ST, (B != 0), VW><<<grid(p.N / VW, 256), 256, 0, a.stream>>>(p);
                     else
@@ -73,6 +105,12 @@ cudaError_t launch(const LaunchArgs& a) {
                     };
                     with_coll([&](auto C_) {
                         constexpr int VW = vec_width<CT, ST, NC>();
+                        if constexpr (B != 0) {
+                            if (a.list) {
+                                k_step_v<L, NC, CT, ST, C_, true, 1, true><<<grid(p.nfluid, 128), 128, 0, a.stream>>>(p);
+                                return;
+                            }
+                        }
                         if (a.vec == VW && VW > 1)
                             k_step_v<L, NC, CT, ST, C_, (B != 0), VW><<<grid(p.N / VW, 128), 128, 0, a.stream>>>(p);
                         else
@@ -113,6 +151,44 @@ cudaError_t launch(const LaunchArgs& a) {
         case OP_IMPORT_POP: {
             const FieldIO<CT>& io = *static_cast<const FieldIO<CT>*>(a.a0);
             k_import_pop<L, CT, ST><<<grid(io.cnt, 256), 256, 0, a.stream>>>(p, a.i0, io, a.a2);
+            break;
+        }
+        case OP_FUSED: {
+            bool done = false;
+            with_nc([&](auto NC) {
+                auto with_coll = [&](auto fn) {
+                    if (a.coll == 0) fn(IC<0>{});
+                    else if (a.coll == 1) fn(IC<1>{});
+                };
+                with_coll([&](auto C_) {
+                    auto go = [&](auto VEC, auto WX, auto TY, auto PF) {
+                        using T = FusedTile<L, NC, CT, VEC, WX, TY>;
+                        dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), 1, 1);
+                        if (L::D == 3) {
+                            g.y = (unsigned)((p.ny + TY - 1) / TY);
+                            g.z = (unsigned)((p.nz + a.i0 - 1) / a.i0);
+                        } else {
+                            g.y = (unsigned)((p.ny + a.i0 - 1) / a.i0);
+                        }
+                        k_fused_v<L, NC, CT, ST, C_, VEC, WX, TY, (PF != 0)><<<g, T::THREADS, 0, a.stream>>>(p, a.i0);
+                        done = true;
+                    };
+                    constexpr FusedShape fs = fused_shape<L, CT, ST, NC>();
+                    if constexpr (fs.vec > 0) {
+#ifdef LBM_FUSED_TUNING
+                        if constexpr (L::D == 3 && sizeof(CT) == 4 && NC == 1 && C_ == 0) {
+                            static_for<1, FUSED_TUNING_VARIANTS + 1>([&](auto V) {
+                                constexpr FusedShape ts = fused_tuning_shape(V);
+                                if (a.variant == V) go(IC<ts.vec>{}, IC<ts.wx>{}, IC<ts.ty>{}, IC<(fused_tuning_pf(V) ? 1 : 0)>{});
+                            });
+                            if (done) return;
+                        }
+#endif
+                        go(IC<fs.vec>{}, IC<fs.wx>{}, IC<fs.ty>{}, IC<1>{});
+                    }
+                });
+            });
+            if (!done) return cudaErrorInvalidValue;
             break;
         }
         default:

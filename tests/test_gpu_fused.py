@@ -1,0 +1,109 @@
+"""GPU parity of the one-pass kernel K2F (lbm_fused.cuh) against the oracle and against the two-pass path.
+
+K2F recomputes rho -> psi of the ring around its tile instead of reading a psi field written by K1, so the
+cases here stress what is new: tiles with ragged edges in x and y, several marching chunks, wrap-around of
+the ring columns and rows, domains smaller than one tile, both lattices, all dtype combinations it is built
+for, two components, MRT and both forcing schemes.  Gates are those of test_gpu_parity.py.
+"""
+import numpy as np
+import pytest
+
+from conftest import make_oracle
+from paper_2506_17713_b200 import workloads as W
+from test_gpu_parity import TOL16, TOL32, TOL64, assert_parity, make_gpu, small_inputs, with_dtype
+
+pytestmark = pytest.mark.gpu
+
+
+def one_pass(wl):
+    w = dict(wl)
+    w["path"] = "one_pass"
+    return w
+
+
+def run_three(wl, inp, steps, oracle_wl=None):
+    """oracle, K2F and the two-pass path on the same inputs; returns populations of each."""
+    o = make_oracle(oracle_wl or wl, inp)
+    g1 = make_gpu(one_pass(wl), inp)
+    g2 = make_gpu(dict(wl, path="two_pass"), inp)
+    o.step(steps)
+    l0 = g1.kernel_launches
+    g1.step(steps)
+    assert g1.kernel_launches - l0 == steps      # one launch per step: K2F ran, not K1 + K2
+    g2.step(steps)
+    return ([o.get_populations(k) for k in range(o.nc)], [g1.get_populations(k) for k in range(o.nc)],
+            [g2.get_populations(k) for k in range(o.nc)], o)
+
+
+@pytest.mark.parametrize("dims", [(128, 24, 20), (132, 9, 11), (4, 3, 2), (260, 8, 5), (8, 35, 3)])
+def test_d3q19_fp64_ragged_tiles(dims, monkeypatch):
+    monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "7")   # several marching chunks, ragged last one
+    wl, _ = W.config5(16, "f64")
+    wl.update(nx=dims[0], ny=dims[1], nz=dims[2])
+    inp = small_inputs(wl, 21, 0.05, 0.3)
+    fo, f1, f2, o = run_three(wl, inp, 30)
+    fluid = np.ones(o.N, bool)
+    assert_parity(fo, f1, fluid, TOL64, relative=False)
+    assert_parity(f2, f1, fluid, 1e-13, relative=False)   # same arithmetic in the same order as K2
+
+
+def test_config5_fp32_100_steps():
+    wl, inp = W.config5(48, "f32")
+    fo, f1, f2, o = run_three(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
+    fluid = np.ones(o.N, bool)
+    assert_parity(fo, f1, fluid, TOL32, relative=True)
+    assert_parity(f2, f1, fluid, 2e-6, relative=True)
+
+
+def test_config5_fp16_storage():
+    wl, inp = W.config5(32, "f32", store_dtype="f16")
+    fo, f1, f2, o = run_three(wl, inp, 100)   # the oracle emulates the fp16 rounding at the store (R16)
+    fluid = np.ones(o.N, bool)
+    assert_parity(fo, f1, fluid, TOL16, relative=True)
+
+
+def test_config3_mrt_peng_robinson_fp64():
+    wl, _ = W.config3(20, "f64")
+    wl.update(nx=24, ny=19, nz=17)
+    inp = small_inputs(wl, 3, 3.9, 4.2)
+    fo, f1, f2, o = run_three(wl, inp, 100)
+    assert_parity(fo, f1, np.ones(o.N, bool), TOL64, relative=False)
+
+
+@pytest.mark.parametrize("nx,ny", [(64, 64), (70, 37), (200, 3), (2, 5)])
+def test_d2q9_fp64(nx, ny, monkeypatch):
+    monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "9")
+    wl, _ = W.config1(8, "f64")
+    wl.update(nx=nx, ny=ny)
+    inp = small_inputs(wl, 11, 0.05, 0.25)
+    fo, f1, f2, o = run_three(wl, inp, 100)
+    assert_parity(fo, f1, np.ones(o.N, bool), TOL64, relative=False)
+
+
+@pytest.mark.parametrize("lattice,n", [("D2Q9", (46, 23, 1)), ("D3Q19", (22, 10, 9))])
+@pytest.mark.parametrize("collision", ["BGK", "MRT"])
+@pytest.mark.parametrize("forcing", ["EDM", "SHIFT"])
+def test_two_components_variants_fp32(lattice, n, collision, forcing):
+    g = 3.5 / 3.0
+    wl = dict(name="x", lattice=lattice, nx=n[0], ny=n[1], nz=n[2], n_components=2, periodic=(True, True, True),
+              psi_kind=["SC93", "RHO"], eos=[dict(rho0=1.0), dict()], G=[[-0.3, g * 0.4], [g * 0.4, 0.0]],
+              collision=collision, tau=[0.8, 1.3], forcing=forcing, compute_dtype="f32", store_dtype="f32")
+    if collision == "MRT":
+        wl["mrt_rates"] = [W.mrt_rates(lattice, 0.8), W.mrt_rates(lattice, 1.3)]
+    inp = small_inputs(wl, 5, 0.4, 0.9)
+    fo, f1, f2, o = run_three(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
+    assert_parity(fo, f1, np.ones(o.N, bool), TOL32, relative=True)
+
+
+def test_one_pass_refused_where_it_does_not_apply():
+    from paper_2506_17713_b200 import binding
+    wl, inp = W.config2(64, 32, "f32", wall=3)          # solid plates
+    s = make_gpu(one_pass(wl), inp)
+    with pytest.raises(binding.LBMError):
+        s.step(1)
+    wl, inp = W.config5(16, "f32")
+    wl.update(nx=18)                                     # nx not a multiple of the vector width
+    inp = small_inputs(wl, 1)
+    s = make_gpu(one_pass(wl), inp)
+    with pytest.raises(binding.LBMError):
+        s.step(1)
