@@ -51,6 +51,10 @@ struct lbm {
     double face_rho[6][2], face_u[6][3];
     int64_t steps, launches;
     std::string err;
+    // kernel parameter block, rebuilt only when the configuration-derived part changes (params_valid = false)
+    bool params_valid;
+    KParams<float> pf32;
+    KParams<double> pf64;
     // measurement only (lbm_set_profiling): event pairs around hot-loop kernels
     bool profiling;
     std::vector<cudaEvent_t> ev_pool;
@@ -433,19 +437,30 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.list = (h->use_list && (op == OP_MOMENTS || op == OP_STEP)) ? 1 : 0;
     a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
     a.variant = h->fvariant;
+    a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;
+    a.pfd = 0;
+    if (const char* e = std::getenv("LBM_TUNE_FUSED_PFD")) a.pfd = std::atoi(e);
     a.stream = h->stream;
     launch_fn fn = pick_launch(h->cfg);
     if (!fn) return fail(h, LBM_E_UNSUPPORTED, "dtype combination not built");
     cudaError_t e;
-    if (h->cfg.compute_dtype == LBM_F32) {
-        KParams<float> p = make_params<float>(h, in_buf, out_buf);
-        a.params = &p;
-        e = fn(a);
-    } else {
-        KParams<double> p = make_params<double>(h, in_buf, out_buf);
-        a.params = &p;
-        e = fn(a);
+    if (!h->params_valid) {
+        if (h->cfg.compute_dtype == LBM_F32) h->pf32 = make_params<float>(h, 0, 1);
+        else h->pf64 = make_params<double>(h, 0, 1);
+        h->params_valid = true;
     }
+    // per-launch fields
+    auto patch = [&](auto& p) {
+        p.f_in = h->ws + h->cv.f[in_buf];
+        p.f_out = h->ws + h->cv.f[out_buf];
+        p.nbsolid = h->nbsolid;
+        p.nfluid = h->nfluid;
+        p.write_rho = (h->nbsolid > 0 || h->force_rho) ? 1 : 0;
+        a.params = &p;
+    };
+    if (h->cfg.compute_dtype == LBM_F32) patch(h->pf32);
+    else patch(h->pf64);
+    e = fn(a);
     if (e != cudaSuccess) return cuda_fail(h, e, "kernel launch");
     if (!(op == OP_VIRTUAL && h->nbsolid == 0)) h->launches++;
     return LBM_OK;
@@ -467,7 +482,7 @@ FusedShape fused_shape_of(const lbm_config_t& c, int variant) {
     auto pick = [&](auto L) -> FusedShape {
         using LT = decltype(L);
         const bool f32 = c.compute_dtype == LBM_F32;
-        if (variant > 0) {
+        if (variant > 0 && variant != 11) {
 #ifdef LBM_FUSED_TUNING
             if (LT::D == 3 && f32 && c.n_components == 1 && c.collision == LBM_BGK && variant <= FUSED_TUNING_VARIANTS)
                 return fused_tuning_shape(variant);
@@ -486,6 +501,8 @@ void plan_fused(lbm* h) {
     const lbm_config_t& c = h->cfg;
     if (c.flags & (LBM_FLAG_TWO_PASS | LBM_FLAG_NO_COLLIDE)) return;
     if (h->bnd || h->fshape.vec == 0 || c.nx % h->fshape.vec != 0) return;
+    if ((unsigned long long)c.n_components * h->q * (unsigned long long)h->plane >= (1ULL << 32)) return;   // 32-bit element offsets
+    if (h->d == 3 && c.nx % (16 / (int)h->sbytes) != 0 && h->fvariant == 0) h->fvariant = -1;   // k_fused_ws copies 16-byte pads
     const int nm = h->d == 3 ? c.nz : c.ny;
     const int tx = h->fshape.wx * 32 * h->fshape.vec;
     const long long tiles = (long long)((c.nx + tx - 1) / tx) * (h->d == 3 ? (c.ny + h->fshape.ty - 1) / h->fshape.ty : 1);
@@ -557,6 +574,7 @@ int prepare(lbm* h) {
         }
     }
     h->dirty = false;
+    h->params_valid = false;
     plan_fused(h);
     return LBM_OK;
 }
@@ -652,6 +670,7 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
         if (v < 1) v = 1;
         if (cfg->nx % v == 0) h->vec = v;
     }
+    h->params_valid = false;
     h->fvariant = 0;
     if (const char* e = std::getenv("LBM_TUNE_FUSED_VARIANT")) h->fvariant = std::atoi(e);
     h->fshape = fused_shape_of(*cfg, h->fvariant);

@@ -1,0 +1,382 @@
+// lbm_fused_ws.cuh -- K2F for D3Q19: the one-pass hot kernel as a warp-specialised producer / consumer pipeline.
+//
+//   k_fused_ws   S1 (rho, j) + S3 (psi) + S4..S7 in ONE pass over the populations
+//                Eq. 4/10, Eq. 12, Eq. 13, Eq. 3, Eq. 5, Eq. 2
+//
+// Same idea as k_fused_v (lbm_fused.cuh): a CTA owns an x-y tile of TX x TY cells, marches along z, and recomputes
+// rho -> psi of the one-cell ring around the tile from the populations, so that the populations cross HBM once per
+// step (B1 = 2 q s bytes per cell instead of B2 = 3 q s + 2 c).  The lock-step version is bound by
+// instruction issue and by its phases (load, barrier, collide) not overlapping.  Here the two halves of the step
+// run concurrently on different planes:
+//
+//   producers (one warp per tile row incl. the two halo rows, VEC cells per lane, + two warps for the ring columns)
+//       plane p: copy the row segments the pull needs (S7 read side: 19 source rows, one per direction, each with one
+//       vector of padding where the pull is shifted in x) from global memory straight into a 2-deep stage in shared
+//       memory with cp.async (LDGSTS): the whole plane-row is in flight at once and costs no registers.  Then sum
+//       rho from the stage, evaluate psi -> psi ring in shared memory (5 planes).
+//   consumers (one warp per interior row)
+//       plane m: take the pulled populations from the stage into registers, release the stage, wait for psi of
+//       plane m+1, then moments, force from the psi planes m-1, m, m+1, collision, store (S7 write side).
+//
+//   Hand-over is by mbarriers in shared memory (full / empty per stage, one "psi ready" barrier per ring slot).
+//   Producers need few registers, consumers hold Q x VEC values: the register file is re-split with setmaxnreg
+//   after the role dispatch.  A first version loaded through registers: ptxas split the 29 loads of a plane-row into
+//   ~12 batches and the producers paid the memory latency once per batch (profiles/): hence the asynchronous copies.
+//   Addresses are 32-bit element offsets scaled onto per-thread 64-bit bases (mad.wide.u32): two instructions per
+//   access instead of five.
+// Arithmetic (order of every sum) is that of K1 / K2 in lbm_hot.cuh.
+#pragma once
+#include "lbm_hot.cuh"
+
+namespace lbmk {
+
+// ------------------------------------------------------------------ mbarrier / register-split primitives (PTX)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n"
+        "W%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "\t@p bra D%=;\n\tbra W%=;\n"
+        "D%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+
+// base + idx * sizeof(T) with a 32-bit element index: one IMAD.WIDE.U32
+template <class T>
+__device__ __forceinline__ const T* at_u32(const T* base, unsigned idx) {
+    const T* r;
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(idx), "n"((int)sizeof(T)), "l"(base));
+    return r;
+}
+template <class T>
+__device__ __forceinline__ T* at_u32(T* base, unsigned idx) {
+    T* r;
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(idx), "n"((int)sizeof(T)), "l"(base));
+    return r;
+}
+
+// asynchronous global -> shared copy of BYTES (4, 8 or 16) per thread
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
+    if constexpr (BYTES == 16)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+}
+
+template <class L, int NC, class CT, class ST, int VEC, int TY>
+struct WsTile {
+    static_assert(L::D == 3, "the warp-specialised kernel marches along z");
+    static_assert(TY % 4 == 0, "consumer warps come in warpgroups of four (setmaxnreg)");
+    static constexpr int Q = L::Q;
+    static constexpr int ROWS = TY + 2;
+    static constexpr int TX = 32 * VEC;
+    static constexpr int PAD = 16 / (int)sizeof(CT);               // psi rows: cells left / right of the tile
+    static constexpr int PITCH = TX + 2 * PAD;
+    static constexpr int PADS = 16 / (int)sizeof(ST);              // stage rows: one 16-byte vector left / right
+    static constexpr int PITCHS = TX + 2 * PADS;
+    static constexpr int NS = 5;                                   // psi ring slots (>= 5, see the hand-over notes)
+    static constexpr int NCONS = TY;                               // consumer warps
+    static constexpr int NPROD = (ROWS + 2 + 3) / 4 * 4;           // row producers + 2 ring warps, whole warpgroups
+    static constexpr int THREADS = (NCONS + NPROD) * 32;
+    static constexpr size_t ROW_ELEMS = (size_t)NC * Q * PITCHS;                    // one tile row, all directions
+    static constexpr size_t STAGE_ELEMS = ROW_ELEMS * TY;                           // one stage (interior rows)
+    static constexpr size_t PSI_ELEMS = (size_t)NS * NC * ROWS * PITCH;
+    static constexpr size_t SMEM = sizeof(ST) * (2 * STAGE_ELEMS + 2 * ROW_ELEMS) + sizeof(CT) * PSI_ELEMS + 8 * (4 + NS);
+    // register split: the pool is THREADS x (registers at launch)
+    static constexpr int REG_LAUNCH = (65536 / THREADS) / 8 * 8;
+    static constexpr int REG_PROD = 56;
+    static constexpr int REG_CONS = ((REG_LAUNCH * THREADS - REG_PROD * NPROD * 32) / (NCONS * 32)) / 8 * 8;
+    static_assert(SMEM <= 227 * 1024, "tile does not fit shared memory");
+    static_assert(ROWS <= 32, "ring warps map one lane to one row");
+    static_assert((VEC * sizeof(ST)) % 4 == 0 && VEC * sizeof(ST) <= 16, "per-lane copy size");
+};
+
+// One pulled vector from a staged row: f[v] = row_i[x_v - e_x] for the thread's VEC cells (row points at the lane's
+// first cell; the pads hold the neighbouring vectors of the tile edges)
+template <class CT, class ST, int VEC, int EX>
+__device__ __forceinline__ void pulled_from_row(const ST* row, CT (&f)[VEC]) {
+    using R = typename RawVec<sizeof(ST) * VEC>::type;
+    const R raw = *reinterpret_cast<const R*>(row);
+    const ST* tv = reinterpret_cast<const ST*>(&raw);
+    if constexpr (EX == 0) {
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) f[v] = Cvt<CT, ST>::up(tv[v]);
+    } else if constexpr (EX > 0) {
+        f[0] = Cvt<CT, ST>::up(row[-1]);
+#pragma unroll
+        for (int v = 1; v < VEC; ++v) f[v] = Cvt<CT, ST>::up(tv[v - 1]);
+    } else {
+#pragma unroll
+        for (int v = 0; v < VEC - 1; ++v) f[v] = Cvt<CT, ST>::up(tv[v + 1]);
+        f[VEC - 1] = Cvt<CT, ST>::up(row[VEC]);
+    }
+}
+
+template <class L, int NC, class CT, class ST, int COLL, int VEC, int TY, bool WREF, bool PF>
+__global__ void __launch_bounds__((WsTile<L, NC, CT, ST, VEC, TY>::THREADS), 1)
+k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
+    using T = WsTile<L, NC, CT, ST, VEC, TY>;
+    constexpr int Q = L::Q;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    ST* stage = reinterpret_cast<ST*>(smem_raw);                        // [2][TY][NC][Q][PITCHS]
+    ST* halo = stage + 2 * T::STAGE_ELEMS;                              // [2][NC][Q][PITCHS] landing rows of the halo producers
+    CT* psi_s = reinterpret_cast<CT*>(halo + 2 * T::ROW_ELEMS);         // [NS][NC][ROWS][PITCH]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(psi_s + T::PSI_ELEMS); // full[2], empty[2], psi_ready[NS]
+    uint64_t* bar_full = bars;
+    uint64_t* bar_empty = bars + 2;
+    uint64_t* bar_psi = bars + 4;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < 2; ++s) { mbar_init(bar_full + s, TY); mbar_init(bar_empty + s, T::NCONS); }
+        for (int s = 0; s < T::NS; ++s) mbar_init(bar_psi + s, T::NPROD);
+    }
+    __syncthreads();
+
+    const int tx0 = blockIdx.x * T::TX;
+    const int txw = min(T::TX, p.nx - tx0);
+    const int yb = blockIdx.y * TY;
+    const int nint = min(TY, p.ny - yb);                 // interior rows of this tile
+    const int nm = p.nz;
+    const unsigned sy = (unsigned)p.nx, sz = (unsigned)p.nx * (unsigned)p.ny;
+    const int m0 = blockIdx.z * mchunk, m1 = min(nm, m0 + mchunk);
+    const unsigned plane = (unsigned)p.plane;
+    auto wrap_y = [&](int y) { return y < 0 ? y + p.ny : (y >= p.ny ? y - p.ny : y); };
+    auto wrap_m = [&](int m) { return m < 0 ? m + nm : (m >= nm ? m - nm : m); };
+    auto psi_row = [&](int slot, int k, int r) { return psi_s + ((size_t)(slot * NC + k) * T::ROWS + r) * T::PITCH; };
+
+    if (warp < T::NCONS) {
+        // =============================================================== consumers
+        reg_inc<T::REG_CONS>();
+        const int cw = warp;               // interior row index 0..TY-1  (tile row r = cw + 1)
+        const int xl = lane * VEC;
+        const bool act = cw < nint && xl < txw;
+        const int yw = wrap_y(yb + cw);
+        const unsigned cell0 = (unsigned)yw * sy + (unsigned)(tx0 + xl);
+        for (int m = m0; m < m1; ++m) {
+            const int it = m - m0, s = it & 1;
+            mbar_wait(bar_full + s, (it >> 1) & 1);
+            CT A[NC][Q][VEC];
+            if (act) {
+                const ST* rows = stage + (size_t)s * T::STAGE_ELEMS + (size_t)cw * T::ROW_ELEMS + T::PADS + xl;
+#pragma unroll
+                for (int k = 0; k < NC; ++k)
+                    static_for<0, Q>([&](auto I) {
+                        constexpr int i = I;
+                        pulled_from_row<CT, ST, VEC, L::E[i][0]>(rows + (k * Q + i) * T::PITCHS, A[k][i]);
+                    });
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty + s);
+            if constexpr (PF) {
+                // optional L2 prefetch of plane m + pfd of this row (the edge consumers also the halo rows)
+                const int mp = m + pfd;
+                if (pfd > 0 && mp <= m1 && xl < txw && cw < nint) {
+                    const unsigned zq[3] = {(unsigned)wrap_m(mp - 1) * sz, (unsigned)wrap_m(mp) * sz, (unsigned)wrap_m(mp + 1) * sz};
+                    const ST* bC = static_cast<const ST*>(p.f_in) + (tx0 + xl);
+                    auto pf_row = [&](int y) {
+                        const unsigned yq[3] = {(unsigned)wrap_y(y - 1) * sy, (unsigned)y * sy, (unsigned)wrap_y(y + 1) * sy};
+#pragma unroll
+                        for (int k = 0; k < NC; ++k)
+                            static_for<0, Q>([&](auto I) {
+                                constexpr int i = I;
+                                const unsigned idx = (unsigned)(k * Q + i) * plane + zq[1 - L::E[i][2]] + yq[1 - L::E[i][1]];
+                                asm volatile("prefetch.global.L2 [%0];" ::"l"(at_u32(bC, idx)));
+                            });
+                    };
+                    pf_row(yw);
+                    if (cw == 0) pf_row(wrap_y(yb - 1));
+                    if (cw == nint - 1) pf_row(wrap_y(yb + nint));
+                }
+            }
+            // psi of planes m-1, m, m+1: plane q (counted from m0-1) lives in slot q % NS
+            const int qn = it + 2;
+            mbar_wait(bar_psi + (qn % T::NS), (qn / T::NS) & 1);
+            if (!act) continue;
+            const int sc = (it + 1) % T::NS;
+            CT S[NC][3][VEC], pc[NC][VEC];
+            if constexpr (COLL != 2) {
+#pragma unroll
+                for (int kp = 0; kp < NC; ++kp) {
+                    psi_sums_rows<L, CT, VEC>(
+                        [&](auto DY, auto DZ, auto NX, CT (&t)[VEC], CT& left, CT& right) {
+                            const CT* row = psi_row((sc + DZ + T::NS) % T::NS, kp, cw + 1 + DY) + T::PAD + xl;
+                            using R = typename RawVec<sizeof(CT) * VEC>::type;
+                            const R raw = *reinterpret_cast<const R*>(row);
+                            const CT* tv = reinterpret_cast<const CT*>(&raw);
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v) t[v] = tv[v];
+                            if constexpr (NX != 0) { left = row[-1]; right = row[VEC]; }
+                        },
+                        S[kp], pc[kp]);
+                }
+            }
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                CT fc[NC][Q];
+#pragma unroll
+                for (int k = 0; k < NC; ++k)
+                    static_for<0, Q>([&](auto I) {
+                        if constexpr (WREF) fc[k][I] = A[k][I][v] + p.wref[I];
+                        else fc[k][I] = A[k][I][v];
+                    });
+                if constexpr (COLL != 2) {
+                    CT rc[NC], jc[NC][3], Sc[NC][3], pcc[NC], uc[3], duc[NC][3];
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) {
+                        moments<L, CT>(fc[k], rc[k], jc[k]);
+                        pcc[k] = pc[k][v];
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) Sc[k][a] = S[k][a][v];
+                    }
+                    force_and_velocity<NC, CT>(p, rc, jc, Sc, pcc, uc, duc);
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) collide<L, COLL, CT>(p, k, rc[k], uc, duc[k], fc[k]);
+                }
+#pragma unroll
+                for (int k = 0; k < NC; ++k)
+                    static_for<0, Q>([&](auto I) {
+                        if constexpr (WREF) A[k][I][v] = fc[k][I] - p.wref[I];
+                        else A[k][I][v] = fc[k][I];
+                    });
+            }
+            ST* po = at_u32(static_cast<ST*>(p.f_out), (unsigned)wrap_m(m) * sz + cell0);
+#pragma unroll
+            for (int k = 0; k < NC; ++k)
+                static_for<0, Q>([&](auto I) {
+                    st_vec<CT, ST, VEC>(po + (size_t)(k * Q + I) * plane, A[k][I]);
+                });
+        }
+    } else {
+        // =============================================================== producers
+        reg_dec<T::REG_PROD>();
+        const int pw = warp - T::NCONS;
+        const ST* fin = static_cast<const ST*>(p.f_in);
+        if (pw < T::ROWS) {
+            // ---- row producer: tile row r (0 and nint+1 are the halo rows)
+            const int r = pw;
+            const int xl = lane * VEC;
+            const bool used = r <= nint + 1;
+            const bool act = used && xl < txw;
+            const bool interior = r >= 1 && r <= nint;
+            const bool lastlane = xl + VEC == txw;
+            const int yw = wrap_y(yb - 1 + r);
+            // the 16-byte vectors just left / right of the tile (periodic wrap), copied by lane 0 / the last lane
+            const int xlp = (tx0 > 0 ? tx0 : p.nx) - T::PADS;
+            const int xrp = tx0 + txw < p.nx ? tx0 + txw : 0;
+            const ST* bC = fin + (tx0 + xl);
+            const ST* bP = fin + (lane == 0 ? xlp : xrp);
+            const unsigned yo[3] = {(unsigned)wrap_y(yw - 1) * sy, (unsigned)yw * sy, (unsigned)wrap_y(yw + 1) * sy};
+            for (int pl = m0 - 1; pl <= m1; ++pl) {
+                const int it = pl - m0;                       // -1 .. mchunk
+                const bool staged = it >= 0 && pl < m1;       // planes m0-1 and m1 only feed psi
+                const int s = it & 1;
+                if (it >= 0) mbar_wait(bar_empty + s, ((it >> 1) & 1) ^ 1);
+                const int q = it + 1, slot = q % T::NS;
+                // interior rows land in stage s (free: see the wait above; plane m0-1 uses stage 1 before anyone else)
+                ST* land = interior ? stage + (size_t)s * T::STAGE_ELEMS + (size_t)(r - 1) * T::ROW_ELEMS
+                                    : halo + (r == 0 ? 0 : T::ROW_ELEMS);
+                if (act) {
+                    const unsigned zo[3] = {(unsigned)wrap_m(pl - 1) * sz, (unsigned)wrap_m(pl) * sz, (unsigned)wrap_m(pl + 1) * sz};
+#pragma unroll
+                    for (int k = 0; k < NC; ++k)
+                        static_for<0, Q>([&](auto I) {
+                            constexpr int i = I;
+                            constexpr int ex = L::E[i][0], ey = L::E[i][1], ez = L::E[i][2];
+                            const unsigned idx = (unsigned)(k * Q + i) * plane + zo[1 - ez] + yo[1 - ey];
+                            ST* dst = land + (k * Q + i) * T::PITCHS;
+                            cp_async<VEC * (int)sizeof(ST)>(dst + T::PADS + xl, at_u32(bC, idx));
+                            if constexpr (ex > 0) {
+                                if (lane == 0) cp_async<16>(dst, at_u32(bP, idx));
+                            } else if constexpr (ex < 0) {
+                                if (lastlane) cp_async<16>(dst + T::PADS + txw, at_u32(bP, idx));
+                            }
+                        });
+                }
+                cp_async_wait_all();
+                __syncwarp();
+                if (act) {
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) {
+                        CT rho[VEC], pair[VEC];
+                        static_for<0, Q>([&](auto I) {
+                            constexpr int i = I;
+                            CT f[VEC];
+                            pulled_from_row<CT, ST, VEC, L::E[i][0]>(land + (k * Q + i) * T::PITCHS + T::PADS + xl, f);
+                            if constexpr (WREF) {
+#pragma unroll
+                                for (int v = 0; v < VEC; ++v) f[v] += p.wref[i];
+                            }
+                            // rho in the order of density(): f0 + (f1 + f2) + (f3 + f4) + ...
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v) {
+                                if constexpr (i == 0) rho[v] = f[v];
+                                else if constexpr (i % 2 == 1) pair[v] = f[v];
+                                else rho[v] += pair[v] + f[v];
+                            }
+                        });
+                        CT ps[VEC];
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) ps[v] = psi_of_rho(p, k, rho[v]);
+                        st_vec<CT, CT, VEC>(psi_row(slot, k, r) + T::PAD + xl, ps);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(bar_psi + slot);
+                    if (staged && r >= 1 && r <= TY) mbar_arrive(bar_full + s);
+                }
+            }
+        } else {
+            // ---- ring warps: the columns left (side 0) / right (side 1) of the tile, one lane per tile row
+            const int side = pw - T::ROWS;
+            const int r = lane;
+            const bool act = side < 2 && r <= nint + 1;
+            const int xr = side == 0 ? (tx0 > 0 ? tx0 - 1 : p.nx - 1) : (tx0 + txw < p.nx ? tx0 + txw : 0);
+            const int xrm = xr > 0 ? xr - 1 : p.nx - 1, xrp = xr + 1 < p.nx ? xr + 1 : 0;
+            const ST* b[3] = {fin + xrm, fin + xr, fin + xrp};   // source column for e_x = +1, 0, -1
+            const int yw = wrap_y(yb - 1 + r);
+            const unsigned yo[3] = {(unsigned)wrap_y(yw - 1) * sy, (unsigned)yw * sy, (unsigned)wrap_y(yw + 1) * sy};
+            const int col = side == 0 ? T::PAD - 1 : T::PAD + txw;
+            for (int pl = m0 - 1; pl <= m1; ++pl) {
+                const int it = pl - m0;
+                if (it >= 0) mbar_wait(bar_empty + (it & 1), ((it >> 1) & 1) ^ 1);   // pacing only
+                const int q = it + 1, slot = q % T::NS;
+                if (act) {
+                    const unsigned zo[3] = {(unsigned)wrap_m(pl - 1) * sz, (unsigned)wrap_m(pl) * sz, (unsigned)wrap_m(pl + 1) * sz};
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) {
+                        CT rho = CT(0), pair = CT(0);
+                        static_for<0, Q>([&](auto I) {
+                            constexpr int i = I;
+                            constexpr int ex = L::E[i][0], ey = L::E[i][1], ez = L::E[i][2];
+                            const unsigned idx = (unsigned)(k * Q + i) * plane + zo[1 - ez] + yo[1 - ey];
+                            CT f = ld_one<CT, ST>(at_u32(b[1 - ex], idx));
+                            if constexpr (WREF) f += p.wref[i];
+                            if constexpr (i == 0) rho = f;
+                            else if constexpr (i % 2 == 1) pair = f;
+                            else rho += pair + f;
+                        });
+                        psi_row(slot, k, r)[col] = psi_of_rho(p, k, rho);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_psi + slot);
+            }
+        }
+    }
+}
+
+}  // namespace lbmk

@@ -226,12 +226,14 @@ __device__ __forceinline__ CT density(const CT (&f)[L::Q]) {
     return r;
 }
 
-// acc_i += coef * f_eq,i(rho, u)   (R1: f_eq = w rho [1 + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u]); a pair shares its even part
-template <class L, class CT>
+// acc_i (+)= coef * f_eq,i(rho, u)   (R1: f_eq = w rho [1 + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u]); a pair shares its even part.
+// SET: acc_i = ... (the accumulator is not read)
+template <class L, class CT, bool SET = false>
 __device__ __forceinline__ void add_feq(CT coef, CT rho, const CT (&u)[3], CT (&acc)[L::Q]) {
     const CT cr = coef * rho;
     const CT c0 = CT(1) - CT(1.5) * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
-    acc[0] += (cr * (CT(L::WN[0]) / CT(L::WD))) * c0;
+    if constexpr (SET) acc[0] = (cr * (CT(L::WN[0]) / CT(L::WD))) * c0;
+    else acc[0] += (cr * (CT(L::WN[0]) / CT(L::WD))) * c0;
     static_for<0, (L::Q - 1) / 2>([&](auto P) {
         constexpr int a = 2 * P + 1, b = a + 1;
         constexpr int ex = L::E[a][0], ey = L::E[a][1], ez = L::E[a][2];
@@ -245,8 +247,13 @@ __device__ __forceinline__ void add_feq(CT coef, CT rho, const CT (&u)[3], CT (&
         const CT wr = cr * (CT(L::WN[a]) / CT(L::WD));
         const CT even = c0 + CT(4.5) * eu * eu;
         const CT odd = CT(3) * eu;
-        acc[a] += wr * (even + odd);
-        acc[b] += wr * (even - odd);
+        if constexpr (SET) {
+            acc[a] = wr * (even + odd);
+            acc[b] = wr * (even - odd);
+        } else {
+            acc[a] += wr * (even + odd);
+            acc[b] += wr * (even - odd);
+        }
     });
 }
 
@@ -270,9 +277,15 @@ __device__ __forceinline__ void collide(const KParams<CT>& p, int k, CT rho, con
     }
     if constexpr (COLL == 0) {
         const CT keep = p.c_keep[k], ca = p.c_feq_a[k], cb = p.c_feq_b[k];
-        static_for<0, L::Q>([&](auto I) { f[I] *= keep; });
-        if (ca != CT(0)) add_feq<L, CT>(ca, rho, ua, f);
-        if (cb != CT(0)) add_feq<L, CT>(cb, rho, ub, f);
+        if (keep == CT(0) && ca == CT(0)) {          // tau = 1, EDM: f* = f_eq(rho, u' + du)
+            add_feq<L, CT, true>(cb, rho, ub, f);
+        } else if (keep == CT(0) && cb == CT(0)) {   // tau = 1, SHIFT: f* = f_eq(rho, u' + tau du)
+            add_feq<L, CT, true>(ca, rho, ua, f);
+        } else {
+            static_for<0, L::Q>([&](auto I) { f[I] *= keep; });
+            if (ca != CT(0)) add_feq<L, CT>(ca, rho, ua, f);
+            if (cb != CT(0)) add_feq<L, CT>(cb, rho, ub, f);
+        }
     } else {
         CT e[L::Q];
         static_for<0, L::Q>([&](auto I) { e[I] = CT(0); });

@@ -2,6 +2,7 @@
 // One translation unit per (lattice, compute dtype, storage dtype) instantiates launch<L,CT,ST>.
 #pragma once
 #include "lbm_fused.cuh"
+#include "lbm_fused_ws.cuh"
 
 namespace lbmk {
 
@@ -19,7 +20,10 @@ struct LaunchArgs {
     const void* a1;
     void* a2;
     int i0;              // op-specific integer (OP_FUSED: planes marched per CTA)
-    int variant;         // OP_FUSED: tile variant (0 = default; others are tuning experiments)
+    int variant;         // OP_FUSED: 0 = default (warp-specialised k_fused_ws on D3Q19, lock-step k_fused_v on D2Q9);
+                         //           -1 = lock-step kernel everywhere; 1.. = tuning experiments (LBM_FUSED_TUNING)
+    int pfd;             // OP_FUSED (warp-specialised): L2 prefetch distance in planes
+    int wref;            // OP_FUSED: rho_ref != 0 (populations stored shifted by w_i rho_ref)
     cudaStream_t stream;
 };
 
@@ -174,16 +178,37 @@ cudaError_t launch(const LaunchArgs& a) {
                         done = true;
                     };
                     constexpr FusedShape fs = fused_shape<L, CT, ST, NC>();
-                    if constexpr (fs.vec > 0) {
-#ifdef LBM_FUSED_TUNING
-                        if constexpr (L::D == 3 && sizeof(CT) == 4 && NC == 1 && C_ == 0) {
-                            static_for<1, FUSED_TUNING_VARIANTS + 1>([&](auto V) {
-                                constexpr FusedShape ts = fused_tuning_shape(V);
-                                if (a.variant == V) go(IC<ts.vec>{}, IC<ts.wx>{}, IC<ts.ty>{}, IC<(fused_tuning_pf(V) ? 1 : 0)>{});
-                            });
-                            if (done) return;
+                    // warp-specialised pipeline (D3Q19): needs the dynamic shared memory opt-in and the register pool
+                    // it re-splits with setmaxnreg (a smaller pool would make setmaxnreg.inc wait forever)
+                    auto go_ws = [&](auto VEC, auto TY, auto WREF, auto PF) {
+                        if constexpr (L::D == 3) {
+                            using T = WsTile<L, NC, CT, ST, VEC, TY>;
+                            auto kern = k_fused_ws<L, NC, CT, ST, C_, VEC, TY, (WREF != 0), (PF != 0)>;
+                            static int ready = 0;   // 0 unknown, 1 usable, -1 not usable
+                            if (ready == 0) {
+                                cudaFuncAttributes fa;
+                                bool ok = cudaFuncGetAttributes(&fa, kern) == cudaSuccess &&
+                                          fa.numRegs * T::THREADS >= T::REG_PROD * T::NPROD * 32 + T::REG_CONS * T::NCONS * 32 &&
+                                          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM) == cudaSuccess;
+                                ready = ok ? 1 : -1;
+                                cudaGetLastError();
+                            }
+                            if (ready < 0) return;
+                            dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + TY - 1) / TY),
+                                   (unsigned)((p.nz + a.i0 - 1) / a.i0));
+                            kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0, a.pfd);
+                            done = true;
                         }
-#endif
+                    };
+                    if constexpr (fs.vec > 0) {
+                        if constexpr (L::D == 3) {
+                            if (a.variant == 0 || a.variant == 11) {
+                                const bool pf = a.variant == 0;
+                                if (a.wref) { if (pf) go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{}, IC<1>{}); else go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{}, IC<0>{}); }
+                                else { if (pf) go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<0>{}, IC<1>{}); else go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<0>{}, IC<0>{}); }
+                                if (done) return;
+                            }
+                        }
                         go(IC<fs.vec>{}, IC<fs.wx>{}, IC<fs.ty>{}, IC<1>{});
                     }
                 });

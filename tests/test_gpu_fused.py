@@ -35,9 +35,12 @@ def run_three(wl, inp, steps, oracle_wl=None):
             [g2.get_populations(k) for k in range(o.nc)], o)
 
 
+@pytest.mark.parametrize("kernel", ["warp_specialised", "lock_step"])
 @pytest.mark.parametrize("dims", [(128, 24, 20), (132, 9, 11), (4, 3, 2), (260, 8, 5), (8, 35, 3)])
-def test_d3q19_fp64_ragged_tiles(dims, monkeypatch):
+def test_d3q19_fp64_ragged_tiles(dims, kernel, monkeypatch):
     monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "7")   # several marching chunks, ragged last one
+    if kernel == "lock_step":                           # k_fused_v instead of k_fused_ws (lbm_launch.cuh)
+        monkeypatch.setenv("LBM_TUNE_FUSED_VARIANT", "-1")
     wl, _ = W.config5(16, "f64")
     wl.update(nx=dims[0], ny=dims[1], nz=dims[2])
     inp = small_inputs(wl, 21, 0.05, 0.3)
@@ -47,7 +50,10 @@ def test_d3q19_fp64_ragged_tiles(dims, monkeypatch):
     assert_parity(f2, f1, fluid, 1e-13, relative=False)   # same arithmetic in the same order as K2
 
 
-def test_config5_fp32_100_steps():
+@pytest.mark.parametrize("kernel", ["warp_specialised", "lock_step"])
+def test_config5_fp32_100_steps(kernel, monkeypatch):
+    if kernel == "lock_step":
+        monkeypatch.setenv("LBM_TUNE_FUSED_VARIANT", "-1")
     wl, inp = W.config5(48, "f32")
     fo, f1, f2, o = run_three(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
     fluid = np.ones(o.N, bool)
