@@ -17,6 +17,8 @@ LIB = HERE / "liblbm_b200.so"
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--expt-relaxed-constexpr",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+if os.environ.get("LBM_EXTRA_NVCC_FLAGS"):   # development switches, e.g. -DLBM_WS_TIMING
+    FLAGS += os.environ["LBM_EXTRA_NVCC_FLAGS"].split()
 if os.environ.get("LBM_FUSED_TUNING"):   # also build the K2F tile-shape experiments (lbm_launch.cuh)
     FLAGS.append("-DLBM_FUSED_TUNING")
 

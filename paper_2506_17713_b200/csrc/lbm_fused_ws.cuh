@@ -30,6 +30,17 @@
 
 namespace lbmk {
 
+// Development aid (-DLBM_WS_TIMING): per-role cycle counters accumulated into the (otherwise unused) rho field.
+#ifdef LBM_WS_TIMING
+#define WS_T0() long long t_prev_ = clock64(); long long t_acc_[6] = {0, 0, 0, 0, 0, 0}
+#define WS_TICK(slot) do { const long long t_now_ = clock64(); t_acc_[slot] += t_now_ - t_prev_; t_prev_ = t_now_; } while (0)
+#define WS_FLUSH(base) do { if (lane == 0) { for (int q_ = 0; q_ < 6; ++q_) atomicAdd(reinterpret_cast<unsigned long long*>(p.rho) + (base) + q_, (unsigned long long)t_acc_[q_]); } } while (0)
+#else
+#define WS_T0() do {} while (0)
+#define WS_TICK(slot) do {} while (0)
+#define WS_FLUSH(base) do {} while (0)
+#endif
+
 // ------------------------------------------------------------------ mbarrier / register-split primitives (PTX)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -75,29 +86,56 @@ __device__ __forceinline__ void cp_async_wait_all() {
     asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
 }
 
-template <class L, int NC, class CT, class ST, int VEC, int TY>
+// TY interior rows per tile, NSTG stages.  With two stages producer and consumer are still coupled (the consumer of
+// plane m needs psi of plane m+1, whose producer could only start when the stage of plane m-1 was released): the step
+// period is the mean of their times, not the maximum; a third stage decouples them.
+// bulk asynchronous copy (TMA unit, SASS UBLKCP): `bytes` contiguous bytes global -> shared, 16-byte aligned on both
+// sides, completion counted on an mbarrier (complete_tx)
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+template <class L, int NC, class CT, class ST, int VEC, int TY, int NSTG>
 struct WsTile {
     static_assert(L::D == 3, "the warp-specialised kernel marches along z");
-    static_assert(TY % 4 == 0, "consumer warps come in warpgroups of four (setmaxnreg)");
+    static_assert(NSTG == 2 || NSTG == 3, "two or three stages");
     static constexpr int Q = L::Q;
     static constexpr int ROWS = TY + 2;
     static constexpr int TX = 32 * VEC;
     static constexpr int PAD = 16 / (int)sizeof(CT);               // psi rows: cells left / right of the tile
     static constexpr int PITCH = TX + 2 * PAD;
     static constexpr int PADS = 16 / (int)sizeof(ST);              // stage rows: one 16-byte vector left / right
-    static constexpr int PITCHS = TX + 2 * PADS;
+    // a staged direction row holds the TX cells of the tile row plus one 16-byte vector on the side its pull is
+    // shifted to (left for e_x = +1, right for e_x = -1)
+    static constexpr int dir_pitch(int i) { return TX + (L::E[i][0] != 0 ? PADS : 0); }
+    static constexpr int dir_lead(int i) { return L::E[i][0] > 0 ? PADS : 0; }          // offset of the tile's first cell
+    static constexpr int dir_off(int i) { int o = 0; for (int j = 0; j < i; ++j) o += dir_pitch(j); return o; }
+    static constexpr int RB = dir_off(Q);                                                 // one component of a tile row
     static constexpr int NS = 5;                                   // psi ring slots (>= 5, see the hand-over notes)
-    static constexpr int NCONS = TY;                               // consumer warps
-    static constexpr int NPROD = (ROWS + 2 + 3) / 4 * 4;           // row producers + 2 ring warps, whole warpgroups
-    static constexpr int THREADS = (NCONS + NPROD) * 32;
-    static constexpr size_t ROW_ELEMS = (size_t)NC * Q * PITCHS;                    // one tile row, all directions
+    // warps come in warpgroups of four (setmaxnreg): consumer group = TY row consumers (+ the two ring warps if two
+    // warps are spare there), producer group = ROWS row producers (+ the ring warps otherwise)
+    static constexpr int NCONS = TY;                               // row consumers
+    static constexpr int NCW = (TY + 3) / 4 * 4;                   // warps of the consumer group
+    static constexpr bool RING_IN_CONS = NCW - TY >= 2;
+    static constexpr int RING0 = RING_IN_CONS ? TY : NCW + ROWS;   // first ring warp
+    static constexpr int NPW = (ROWS + (RING_IN_CONS ? 0 : 2) + 3) / 4 * 4;   // warps of the producer group
+    static constexpr int NPSI = ROWS + 2;                          // arrivals per psi plane: row producers + ring warps
+    static constexpr int THREADS = (NCW + NPW) * 32;
+    static constexpr size_t ROW_ELEMS = (size_t)NC * RB;                            // one tile row, all directions
     static constexpr size_t STAGE_ELEMS = ROW_ELEMS * TY;                           // one stage (interior rows)
     static constexpr size_t PSI_ELEMS = (size_t)NS * NC * ROWS * PITCH;
-    static constexpr size_t SMEM = sizeof(ST) * (2 * STAGE_ELEMS + 2 * ROW_ELEMS) + sizeof(CT) * PSI_ELEMS + 8 * (4 + NS);
+    static constexpr size_t SMEM = sizeof(ST) * (NSTG * STAGE_ELEMS + 4 * ROW_ELEMS) + sizeof(CT) * PSI_ELEMS + 8 * (2 * NSTG + NS + 2 * ROWS);
     // register split: the pool is THREADS x (registers at launch)
     static constexpr int REG_LAUNCH = (65536 / THREADS) / 8 * 8;
     static constexpr int REG_PROD = 56;
-    static constexpr int REG_CONS = ((REG_LAUNCH * THREADS - REG_PROD * NPROD * 32) / (NCONS * 32)) / 8 * 8;
+    static constexpr int REG_CONS_ = ((REG_LAUNCH * THREADS - REG_PROD * NPW * 32) / (NCW * 32)) / 8 * 8;
+    static constexpr int REG_CONS = REG_CONS_ > 208 ? 208 : REG_CONS_;
     static_assert(SMEM <= 227 * 1024, "tile does not fit shared memory");
     static_assert(ROWS <= 32, "ring warps map one lane to one row");
     static_assert((VEC * sizeof(ST)) % 4 == 0 && VEC * sizeof(ST) <= 16, "per-lane copy size");
@@ -124,24 +162,26 @@ __device__ __forceinline__ void pulled_from_row(const ST* row, CT (&f)[VEC]) {
     }
 }
 
-template <class L, int NC, class CT, class ST, int COLL, int VEC, int TY, bool WREF, bool PF>
-__global__ void __launch_bounds__((WsTile<L, NC, CT, ST, VEC, TY>::THREADS), 1)
+template <class L, int NC, class CT, class ST, int COLL, int VEC, int TY, int NSTG, bool WREF, bool PF>
+__global__ void __launch_bounds__((WsTile<L, NC, CT, ST, VEC, TY, NSTG>::THREADS), 1)
 k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
-    using T = WsTile<L, NC, CT, ST, VEC, TY>;
+    using T = WsTile<L, NC, CT, ST, VEC, TY, NSTG>;
     constexpr int Q = L::Q;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    ST* stage = reinterpret_cast<ST*>(smem_raw);                        // [2][TY][NC][Q][PITCHS]
-    ST* halo = stage + 2 * T::STAGE_ELEMS;                              // [2][NC][Q][PITCHS] landing rows of the halo producers
-    CT* psi_s = reinterpret_cast<CT*>(halo + 2 * T::ROW_ELEMS);         // [NS][NC][ROWS][PITCH]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(psi_s + T::PSI_ELEMS); // full[2], empty[2], psi_ready[NS]
+    ST* stage = reinterpret_cast<ST*>(smem_raw);                        // [NSTG][TY][NC][RB]
+    ST* halo = stage + NSTG * T::STAGE_ELEMS;                            // [2 planes][2 halo rows][NC][RB] landing rows
+    CT* psi_s = reinterpret_cast<CT*>(halo + 4 * T::ROW_ELEMS);         // [NS][NC][ROWS][PITCH]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(psi_s + T::PSI_ELEMS); // full[NSTG], empty[NSTG], psi_ready[NS]
     uint64_t* bar_full = bars;
-    uint64_t* bar_empty = bars + 2;
-    uint64_t* bar_psi = bars + 4;
+    uint64_t* bar_empty = bars + NSTG;
+    uint64_t* bar_psi = bars + 2 * NSTG;
+    uint64_t* bar_land = bar_psi + T::NS;                               // [2][ROWS] bulk copies of a row producer landed
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < 2; ++s) { mbar_init(bar_full + s, TY); mbar_init(bar_empty + s, T::NCONS); }
-        for (int s = 0; s < T::NS; ++s) mbar_init(bar_psi + s, T::NPROD);
+        for (int s = 0; s < NSTG; ++s) { mbar_init(bar_full + s, TY); mbar_init(bar_empty + s, T::NCONS); }
+        for (int s = 0; s < T::NS; ++s) mbar_init(bar_psi + s, T::NPSI);
+        for (int s = 0; s < 2 * T::ROWS; ++s) mbar_init(bar_land + s, 1);
     }
     __syncthreads();
 
@@ -157,29 +197,70 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
     auto wrap_m = [&](int m) { return m < 0 ? m + nm : (m >= nm ? m - nm : m); };
     auto psi_row = [&](int slot, int k, int r) { return psi_s + ((size_t)(slot * NC + k) * T::ROWS + r) * T::PITCH; };
 
-    if (warp < T::NCONS) {
-        // =============================================================== consumers
-        reg_inc<T::REG_CONS>();
+    const ST* fin = static_cast<const ST*>(p.f_in);
+
+    // ---- ring role: the columns left (side 0) / right (side 1) of the tile, one lane per tile row
+    auto ring_role = [&](int side) {
+        const int r = lane;
+        const bool act = r <= nint + 1;
+        const int xr = side == 0 ? (tx0 > 0 ? tx0 - 1 : p.nx - 1) : (tx0 + txw < p.nx ? tx0 + txw : 0);
+        const int xrm = xr > 0 ? xr - 1 : p.nx - 1, xrp = xr + 1 < p.nx ? xr + 1 : 0;
+        const ST* b[3] = {fin + xrm, fin + xr, fin + xrp};   // source column for e_x = +1, 0, -1
+        const int yw = wrap_y(yb - 1 + r);
+        const unsigned yo[3] = {(unsigned)wrap_y(yw - 1) * sy, (unsigned)yw * sy, (unsigned)wrap_y(yw + 1) * sy};
+        const int col = side == 0 ? T::PAD - 1 : T::PAD + txw;
+        for (int pl = m0 - 1; pl <= m1; ++pl) {
+            const int it = pl - m0;
+            if (it >= 0) mbar_wait(bar_empty + it % NSTG, ((it / NSTG) & 1) ^ 1);   // pacing only
+            const int q = it + 1, slot = q % T::NS;
+            if (act) {
+                const unsigned zo[3] = {(unsigned)wrap_m(pl - 1) * sz, (unsigned)wrap_m(pl) * sz, (unsigned)wrap_m(pl + 1) * sz};
+#pragma unroll
+                for (int k = 0; k < NC; ++k) {
+                    CT rho = CT(0), pair = CT(0);
+                    static_for<0, Q>([&](auto I) {
+                        constexpr int i = I;
+                        constexpr int ex = L::E[i][0], ey = L::E[i][1], ez = L::E[i][2];
+                        const unsigned idx = (unsigned)(k * Q + i) * plane + zo[1 - ez] + yo[1 - ey];
+                        CT f = ld_one<CT, ST>(at_u32(b[1 - ex], idx));
+                        if constexpr (WREF) f += p.wref[i];
+                        if constexpr (i == 0) rho = f;
+                        else if constexpr (i % 2 == 1) pair = f;
+                        else rho += pair + f;
+                    });
+                    psi_row(slot, k, r)[col] = psi_of_rho(p, k, rho);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_psi + slot);
+        }
+    };
+
+    // =============================================================== consumers
+    auto consumer_role = [&]() {
         const int cw = warp;               // interior row index 0..TY-1  (tile row r = cw + 1)
         const int xl = lane * VEC;
         const bool act = cw < nint && xl < txw;
         const int yw = wrap_y(yb + cw);
         const unsigned cell0 = (unsigned)yw * sy + (unsigned)(tx0 + xl);
+        WS_T0();
         for (int m = m0; m < m1; ++m) {
-            const int it = m - m0, s = it & 1;
-            mbar_wait(bar_full + s, (it >> 1) & 1);
+            const int it = m - m0, s = it % NSTG;
+            mbar_wait(bar_full + s, (it / NSTG) & 1);
+            WS_TICK(0);
             CT A[NC][Q][VEC];
             if (act) {
-                const ST* rows = stage + (size_t)s * T::STAGE_ELEMS + (size_t)cw * T::ROW_ELEMS + T::PADS + xl;
+                const ST* rows = stage + (size_t)s * T::STAGE_ELEMS + (size_t)cw * T::ROW_ELEMS + xl;
 #pragma unroll
                 for (int k = 0; k < NC; ++k)
                     static_for<0, Q>([&](auto I) {
                         constexpr int i = I;
-                        pulled_from_row<CT, ST, VEC, L::E[i][0]>(rows + (k * Q + i) * T::PITCHS, A[k][i]);
+                        pulled_from_row<CT, ST, VEC, L::E[i][0]>(rows + k * T::RB + T::dir_off(i) + T::dir_lead(i), A[k][i]);
                     });
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty + s);
+            WS_TICK(1);
             if constexpr (PF) {
                 // optional L2 prefetch of plane m + pfd of this row (the edge consumers also the halo rows)
                 const int mp = m + pfd;
@@ -204,6 +285,7 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
             // psi of planes m-1, m, m+1: plane q (counted from m0-1) lives in slot q % NS
             const int qn = it + 2;
             mbar_wait(bar_psi + (qn % T::NS), (qn / T::NS) & 1);
+            WS_TICK(2);
             if (!act) continue;
             const int sc = (it + 1) % T::NS;
             CT S[NC][3][VEC], pc[NC][VEC];
@@ -252,61 +334,85 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                         else A[k][I][v] = fc[k][I];
                     });
             }
+            WS_TICK(3);
             ST* po = at_u32(static_cast<ST*>(p.f_out), (unsigned)wrap_m(m) * sz + cell0);
 #pragma unroll
             for (int k = 0; k < NC; ++k)
                 static_for<0, Q>([&](auto I) {
-                    st_vec<CT, ST, VEC>(po + (size_t)(k * Q + I) * plane, A[k][I]);
+                    st_vec_global<CT, ST, VEC>(po + (size_t)(k * Q + I) * plane, A[k][I]);
                 });
+            WS_TICK(4);
         }
-    } else {
-        // =============================================================== producers
-        reg_dec<T::REG_PROD>();
-        const int pw = warp - T::NCONS;
-        const ST* fin = static_cast<const ST*>(p.f_in);
-        if (pw < T::ROWS) {
+        WS_FLUSH(0);
+    };
+    // =============================================================== producers
+    auto producer_role = [&](int r) {
+        {
             // ---- row producer: tile row r (0 and nint+1 are the halo rows)
-            const int r = pw;
             const int xl = lane * VEC;
             const bool used = r <= nint + 1;
             const bool act = used && xl < txw;
             const bool interior = r >= 1 && r <= nint;
-            const bool lastlane = xl + VEC == txw;
             const int yw = wrap_y(yb - 1 + r);
             // the 16-byte vectors just left / right of the tile (periodic wrap), copied by lane 0 / the last lane
             const int xlp = (tx0 > 0 ? tx0 : p.nx) - T::PADS;
             const int xrp = tx0 + txw < p.nx ? tx0 + txw : 0;
-            const ST* bC = fin + (tx0 + xl);
-            const ST* bP = fin + (lane == 0 ? xlp : xrp);
-            const unsigned yo[3] = {(unsigned)wrap_y(yw - 1) * sy, (unsigned)yw * sy, (unsigned)wrap_y(yw + 1) * sy};
+            // lane i < Q issues the bulk copies of direction i: source row (y - e_y, z - e_z) of its plane
+            int ex_l = 0, ey_l = 0, ez_l = 0, off_l = 0;
+            static_for<0, Q>([&](auto I) {
+                if (lane == I) { ex_l = L::E[I][0]; ey_l = L::E[I][1]; ez_l = L::E[I][2]; off_l = T::dir_off(I); }
+            });
+            const unsigned base_l = (unsigned)lane * plane + (unsigned)wrap_y(yw - ey_l) * sy;
+            constexpr int NXD = []() { int n = 0; for (int i = 0; i < Q; ++i) n += L::E[i][0] != 0; return n; }();
+            const uint32_t main_bytes = (uint32_t)txw * (uint32_t)sizeof(ST);
+            const uint32_t land_bytes = (uint32_t)NC * ((uint32_t)Q * main_bytes + (uint32_t)NXD * 16u);
+            // where plane pl of this row lands: interior rows in stage (it mod NSTG), halo rows in their own two buffers
+            auto landing = [&](int it) -> ST* {
+                return interior ? stage + (size_t)((it + NSTG) % NSTG) * T::STAGE_ELEMS + (size_t)(r - 1) * T::ROW_ELEMS
+                                : halo + (size_t)(2 * ((it + 1) & 1) + (r == 0 ? 0 : 1)) * T::ROW_ELEMS;
+            };
+            // start the copies of plane pl (after its stage slot has been released by the consumers)
+            auto issue = [&](int pl) {
+                const int it = pl - m0;
+                if (it >= 0) mbar_wait(bar_empty + it % NSTG, ((it / NSTG) & 1) ^ 1);
+                if (!used) return;
+                uint64_t* lb = bar_land + ((it + 1) & 1) * T::ROWS + r;
+                ST* land = landing(it);
+                if (lane == 0) mbar_expect_tx(lb, land_bytes);
+                __syncwarp();
+                if (lane < Q) {
+                    const unsigned idx0 = base_l + (unsigned)wrap_m(pl - ez_l) * sz;
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) {
+                        const ST* src = fin + ((size_t)k * Q * plane + idx0);
+                        ST* dst = land + k * T::RB + off_l;
+                        // the pad vector is contiguous with the row segment unless the tile touches the periodic seam
+                        if (ex_l > 0) {
+                            if (tx0 > 0) bulk_g2s(dst, src + (tx0 - T::PADS), main_bytes + 16u, lb);
+                            else { bulk_g2s(dst + T::PADS, src + tx0, main_bytes, lb); bulk_g2s(dst, src + xlp, 16u, lb); }
+                        } else if (ex_l < 0) {
+                            if (tx0 + txw < p.nx) bulk_g2s(dst, src + tx0, main_bytes + 16u, lb);
+                            else { bulk_g2s(dst, src + tx0, main_bytes, lb); bulk_g2s(dst + txw, src + xrp, 16u, lb); }
+                        } else {
+                            bulk_g2s(dst, src + tx0, main_bytes, lb);
+                        }
+                    }
+                }
+            };
+            WS_T0();
             for (int pl = m0 - 1; pl <= m1; ++pl) {
                 const int it = pl - m0;                       // -1 .. mchunk
                 const bool staged = it >= 0 && pl < m1;       // planes m0-1 and m1 only feed psi
-                const int s = it & 1;
-                if (it >= 0) mbar_wait(bar_empty + s, ((it >> 1) & 1) ^ 1);
+                const int s = (it + NSTG) % NSTG;
+                // (Issuing the copies of plane pl+1 here as well, before summing plane pl, was tried and is slower with two
+                // stages: the slot of pl+1 is only released once the consumers have collided plane pl-2, so the producer
+                // blocks in front of a rho pass whose data has already landed.)
+                issue(pl);
+                WS_TICK(0);
                 const int q = it + 1, slot = q % T::NS;
-                // interior rows land in stage s (free: see the wait above; plane m0-1 uses stage 1 before anyone else)
-                ST* land = interior ? stage + (size_t)s * T::STAGE_ELEMS + (size_t)(r - 1) * T::ROW_ELEMS
-                                    : halo + (r == 0 ? 0 : T::ROW_ELEMS);
-                if (act) {
-                    const unsigned zo[3] = {(unsigned)wrap_m(pl - 1) * sz, (unsigned)wrap_m(pl) * sz, (unsigned)wrap_m(pl + 1) * sz};
-#pragma unroll
-                    for (int k = 0; k < NC; ++k)
-                        static_for<0, Q>([&](auto I) {
-                            constexpr int i = I;
-                            constexpr int ex = L::E[i][0], ey = L::E[i][1], ez = L::E[i][2];
-                            const unsigned idx = (unsigned)(k * Q + i) * plane + zo[1 - ez] + yo[1 - ey];
-                            ST* dst = land + (k * Q + i) * T::PITCHS;
-                            cp_async<VEC * (int)sizeof(ST)>(dst + T::PADS + xl, at_u32(bC, idx));
-                            if constexpr (ex > 0) {
-                                if (lane == 0) cp_async<16>(dst, at_u32(bP, idx));
-                            } else if constexpr (ex < 0) {
-                                if (lastlane) cp_async<16>(dst + T::PADS + txw, at_u32(bP, idx));
-                            }
-                        });
-                }
-                cp_async_wait_all();
-                __syncwarp();
+                const ST* land = landing(it);
+                if (used) mbar_wait(bar_land + ((it + 1) & 1) * T::ROWS + r, ((it + 1) >> 1) & 1);
+                WS_TICK(1);
                 if (act) {
 #pragma unroll
                     for (int k = 0; k < NC; ++k) {
@@ -314,7 +420,7 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                         static_for<0, Q>([&](auto I) {
                             constexpr int i = I;
                             CT f[VEC];
-                            pulled_from_row<CT, ST, VEC, L::E[i][0]>(land + (k * Q + i) * T::PITCHS + T::PADS + xl, f);
+                            pulled_from_row<CT, ST, VEC, L::E[i][0]>(land + k * T::RB + T::dir_off(i) + T::dir_lead(i) + xl, f);
                             if constexpr (WREF) {
 #pragma unroll
                                 for (int v = 0; v < VEC; ++v) f[v] += p.wref[i];
@@ -333,49 +439,27 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                         st_vec<CT, CT, VEC>(psi_row(slot, k, r) + T::PAD + xl, ps);
                     }
                 }
+                WS_TICK(2);
                 __syncwarp();
                 if (lane == 0) {
                     mbar_arrive(bar_psi + slot);
                     if (staged && r >= 1 && r <= TY) mbar_arrive(bar_full + s);
                 }
+                WS_TICK(3);
             }
-        } else {
-            // ---- ring warps: the columns left (side 0) / right (side 1) of the tile, one lane per tile row
-            const int side = pw - T::ROWS;
-            const int r = lane;
-            const bool act = side < 2 && r <= nint + 1;
-            const int xr = side == 0 ? (tx0 > 0 ? tx0 - 1 : p.nx - 1) : (tx0 + txw < p.nx ? tx0 + txw : 0);
-            const int xrm = xr > 0 ? xr - 1 : p.nx - 1, xrp = xr + 1 < p.nx ? xr + 1 : 0;
-            const ST* b[3] = {fin + xrm, fin + xr, fin + xrp};   // source column for e_x = +1, 0, -1
-            const int yw = wrap_y(yb - 1 + r);
-            const unsigned yo[3] = {(unsigned)wrap_y(yw - 1) * sy, (unsigned)yw * sy, (unsigned)wrap_y(yw + 1) * sy};
-            const int col = side == 0 ? T::PAD - 1 : T::PAD + txw;
-            for (int pl = m0 - 1; pl <= m1; ++pl) {
-                const int it = pl - m0;
-                if (it >= 0) mbar_wait(bar_empty + (it & 1), ((it >> 1) & 1) ^ 1);   // pacing only
-                const int q = it + 1, slot = q % T::NS;
-                if (act) {
-                    const unsigned zo[3] = {(unsigned)wrap_m(pl - 1) * sz, (unsigned)wrap_m(pl) * sz, (unsigned)wrap_m(pl + 1) * sz};
-#pragma unroll
-                    for (int k = 0; k < NC; ++k) {
-                        CT rho = CT(0), pair = CT(0);
-                        static_for<0, Q>([&](auto I) {
-                            constexpr int i = I;
-                            constexpr int ex = L::E[i][0], ey = L::E[i][1], ez = L::E[i][2];
-                            const unsigned idx = (unsigned)(k * Q + i) * plane + zo[1 - ez] + yo[1 - ey];
-                            CT f = ld_one<CT, ST>(at_u32(b[1 - ex], idx));
-                            if constexpr (WREF) f += p.wref[i];
-                            if constexpr (i == 0) rho = f;
-                            else if constexpr (i % 2 == 1) pair = f;
-                            else rho += pair + f;
-                        });
-                        psi_row(slot, k, r)[col] = psi_of_rho(p, k, rho);
-                    }
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_psi + slot);
-            }
+            WS_FLUSH(8);
         }
+    };
+
+    // role dispatch; whole warpgroups execute setmaxnreg together
+    if (warp < T::NCW) {
+        reg_inc<T::REG_CONS>();
+        if (warp < T::NCONS) consumer_role();
+        else if (T::RING_IN_CONS && warp >= T::RING0 && warp < T::RING0 + 2) ring_role(warp - T::RING0);
+    } else {
+        reg_dec<T::REG_PROD>();
+        if (warp < T::NCW + T::ROWS) producer_role(warp - T::NCW);
+        else if (!T::RING_IN_CONS && warp >= T::RING0 && warp < T::RING0 + 2) ring_role(warp - T::RING0);
     }
 }
 

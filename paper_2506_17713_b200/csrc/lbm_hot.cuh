@@ -74,6 +74,25 @@ __device__ __forceinline__ void st_vec(ST* __restrict__ p, const CT (&in)[VEC]) 
     *reinterpret_cast<R*>(p) = r;
 }
 
+// same, through an explicit st.global (for addresses whose provenance the compiler cannot see: generic ST otherwise)
+template <class CT, class ST, int VEC>
+__device__ __forceinline__ void st_vec_global(ST* p, const CT (&in)[VEC]) {
+    using R = typename RawVec<sizeof(ST) * VEC>::type;
+    R r;
+    ST* t = reinterpret_cast<ST*>(&r);
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) t[v] = Cvt<CT, ST>::down(in[v]);
+    if constexpr (sizeof(R) == 16) {
+        const uint4 u = *reinterpret_cast<const uint4*>(&r);
+        asm volatile("st.global.v4.b32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(u.x), "r"(u.y), "r"(u.z), "r"(u.w) : "memory");
+    } else if constexpr (sizeof(R) == 8) {
+        const uint2 u = *reinterpret_cast<const uint2*>(&r);
+        asm volatile("st.global.v2.b32 [%0], {%1, %2};" ::"l"(p), "r"(u.x), "r"(u.y) : "memory");
+    } else {
+        *reinterpret_cast<R*>(p) = r;
+    }
+}
+
 // ------------------------------------------------------------------ geometry of a thread's VEC cells
 struct VCell {
     int id0;       // cell index of lane 0

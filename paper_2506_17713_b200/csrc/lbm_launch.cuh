@@ -180,15 +180,15 @@ cudaError_t launch(const LaunchArgs& a) {
                     constexpr FusedShape fs = fused_shape<L, CT, ST, NC>();
                     // warp-specialised pipeline (D3Q19): needs the dynamic shared memory opt-in and the register pool
                     // it re-splits with setmaxnreg (a smaller pool would make setmaxnreg.inc wait forever)
-                    auto go_ws = [&](auto VEC, auto TY, auto WREF, auto PF) {
+                    auto go_ws = [&](auto VEC, auto TY, auto NSTG, auto WREF, auto PF) {
                         if constexpr (L::D == 3) {
-                            using T = WsTile<L, NC, CT, ST, VEC, TY>;
-                            auto kern = k_fused_ws<L, NC, CT, ST, C_, VEC, TY, (WREF != 0), (PF != 0)>;
+                            using T = WsTile<L, NC, CT, ST, VEC, TY, NSTG>;
+                            auto kern = k_fused_ws<L, NC, CT, ST, C_, VEC, TY, NSTG, (WREF != 0), (PF != 0)>;
                             static int ready = 0;   // 0 unknown, 1 usable, -1 not usable
                             if (ready == 0) {
                                 cudaFuncAttributes fa;
                                 bool ok = cudaFuncGetAttributes(&fa, kern) == cudaSuccess &&
-                                          fa.numRegs * T::THREADS >= T::REG_PROD * T::NPROD * 32 + T::REG_CONS * T::NCONS * 32 &&
+                                          fa.numRegs * T::THREADS >= T::REG_PROD * T::NPW * 32 + T::REG_CONS * T::NCW * 32 &&
                                           cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM) == cudaSuccess;
                                 ready = ok ? 1 : -1;
                                 cudaGetLastError();
@@ -202,12 +202,21 @@ cudaError_t launch(const LaunchArgs& a) {
                     };
                     if constexpr (fs.vec > 0) {
                         if constexpr (L::D == 3) {
-                            if (a.variant == 0 || a.variant == 11) {
-                                const bool pf = a.variant == 0;
-                                if (a.wref) { if (pf) go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{}, IC<1>{}); else go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{}, IC<0>{}); }
-                                else { if (pf) go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<0>{}, IC<1>{}); else go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<0>{}, IC<0>{}); }
+                            // default: two stages of 8 rows.  Variant 12 = three stages of 6 rows (one component only: it
+                            // decouples producers and consumers further but the smaller tile re-reads more; measured slower)
+                            if (a.variant == 0) {
+                                if (a.wref) go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<2>{}, IC<1>{}, IC<1>{});
+                                else go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<2>{}, IC<0>{}, IC<1>{});
                                 if (done) return;
                             }
+#ifdef LBM_FUSED_TUNING
+                            if constexpr (NC == 1) {
+                                if (a.variant == 12 && !a.wref) {
+                                    go_ws(IC<fs.vec>{}, IC<6>{}, IC<3>{}, IC<0>{}, IC<1>{});
+                                    if (done) return;
+                                }
+                            }
+#endif
                         }
                         go(IC<fs.vec>{}, IC<fs.wx>{}, IC<fs.ty>{}, IC<1>{});
                     }
