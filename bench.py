@@ -372,6 +372,7 @@ def main():
 
     if rank == 0 and world == 1:
         if not args.no_cpu_baseline:
+            print("[bench] cpu baseline ...", file=sys.stderr, flush=True)
             res, _ = time_oracle(cpu_sample_of(args.workload), 0, 1, budget_s=15.0)
             line["cpu_baseline"] = {k: res[k] for k in ("value", "unit", "cores", "kind", "sample")}
         if args.all_configs is None or args.all_configs:
@@ -379,6 +380,7 @@ def main():
             for name, k in (("C1-64", 2000), ("C2-512", 2000), ("C3-256", 100), ("C4-400-f16", 50), ("C4-400-f32", 50),
                             ("C5-128", 500), ("C5-256", 200), ("C5-384", 100), ("C5-256-f64", 100)):
                 try:
+                    print(f"[bench] {name} ...", file=sys.stderr, flush=True)
                     rr = gpu_run(torch, name, k, 10, None, want_roofline=True, want_e2e=False)
                     w2 = rr["wl"]
                     mlups = w2["n_components"] * rr["N"] * k / (rr["ms"] * 1e-3) / 1e6

@@ -196,6 +196,16 @@ enum lbm_kernel_id {
 LBM_API int lbm_set_profiling(lbm_t* h, int enable);
 LBM_API int lbm_get_kernel_times(lbm_t* h, double* ms_total, int64_t* launches);
 
+/* Which kernels the most recent lbm_step launched (the driver's "is the native path the one that runs" question,
+ * and the tests' check that a fast kernel was not silently replaced by a fallback). */
+enum lbm_path {
+    LBM_PATH_NONE = 0,              /* no step yet */
+    LBM_PATH_TWO_PASS = 1,          /* K1 (+K1b) + K2 */
+    LBM_PATH_ONE_PASS_LOCKSTEP = 2, /* K2F k_fused_v */
+    LBM_PATH_ONE_PASS_WS = 3        /* K2F k_fused_ws (warp-specialised, bulk asynchronous copies) */
+};
+LBM_API int lbm_hot_path(const lbm_t* h);
+
 /* Bookkeeping. */
 LBM_API int64_t lbm_steps_done(const lbm_t* h);
 LBM_API int64_t lbm_kernel_launches(const lbm_t* h); /* kernels launched by this handle so far */

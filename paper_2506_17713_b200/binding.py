@@ -76,6 +76,7 @@ _SIGNATURES = {
     "lbm_get_lattice": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "lbm_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
     "lbm_get_kernel_times": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "lbm_hot_path": (C.c_int, [C.c_void_p]),
     "lbm_steps_done": (C.c_int64, [C.c_void_p]),
     "lbm_kernel_launches": (C.c_int64, [C.c_void_p]),
     "lbm_last_error": (C.c_char_p, [C.c_void_p]),
@@ -334,6 +335,11 @@ class LBM:
         cnt = (C.c_int64 * len(KERNEL_IDS))()
         self._check(self.L.lbm_get_kernel_times(self.h, ms, cnt), "lbm_get_kernel_times")
         return {name: (ms[i], int(cnt[i])) for name, i in KERNEL_IDS.items()}
+
+    @property
+    def hot_path(self) -> str:
+        """What the most recent step() launched: 'two_pass', 'one_pass_lockstep' or 'one_pass_ws'."""
+        return {0: "none", 1: "two_pass", 2: "one_pass_lockstep", 3: "one_pass_ws"}[int(self.L.lbm_hot_path(self.h))]
 
     @property
     def steps_done(self) -> int:

@@ -43,6 +43,7 @@ struct lbm {
     int fvariant;        // tuning variant of K2F (0 = default)
     int fmchunk;         // planes marched per CTA
     bool use_fused;      // decided in prepare()
+    int last_path;       // lbm_hot_path: what the last lbm_step ran
     bool initialized, has_solid, bnd, dirty, force_rho;
     int nbsolid;
     int nfluid;       // fluid cells (masked domains)
@@ -439,6 +440,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.variant = h->fvariant;
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;
     a.pfd = 0;
+    a.used_kernel = op == OP_FUSED ? &h->last_path : nullptr;
     if (const char* e = std::getenv("LBM_TUNE_FUSED_PFD")) a.pfd = std::atoi(e);
     a.stream = h->stream;
     launch_fn fn = pick_launch(h->cfg);
@@ -682,6 +684,7 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     if (h->fshape.vec == 0 && h->fvariant != 0) { h->fvariant = 0; h->fshape = fused_shape_of(*cfg, 0); }
     h->fmchunk = 1;
     h->use_fused = false;
+    h->last_path = LBM_PATH_NONE;
     h->initialized = false;
     h->has_solid = false;
     h->dirty = true;
@@ -812,6 +815,7 @@ int lbm_step(lbm_t* h, int n) {
             if (h->nbsolid > 0 && (rc = hot_launch(h, OP_VIRTUAL, LBM_K_VIRTUAL))) return rc;
         }
         if ((rc = hot_launch(h, OP_STEP, LBM_K_STEP))) return rc;
+        h->last_path = LBM_PATH_TWO_PASS;
         h->cur ^= 1;
         h->steps++;
     }
@@ -999,6 +1003,7 @@ int lbm_get_lattice(int lattice, int* q, int* e, double* w, int* opposite_out) {
     return LBM_OK;
 }
 
+int lbm_hot_path(const lbm_t* h) { return h ? h->last_path : LBM_E_INVALID; }
 int64_t lbm_steps_done(const lbm_t* h) { return h ? h->steps : LBM_E_INVALID; }
 int64_t lbm_kernel_launches(const lbm_t* h) { return h ? h->launches : LBM_E_INVALID; }
 const char* lbm_last_error(const lbm_t* h) { return h ? h->err.c_str() : "null handle"; }

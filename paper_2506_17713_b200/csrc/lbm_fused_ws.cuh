@@ -255,7 +255,10 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                 for (int k = 0; k < NC; ++k)
                     static_for<0, Q>([&](auto I) {
                         constexpr int i = I;
-                        pulled_from_row<CT, ST, VEC, L::E[i][0]>(rows + k * T::RB + T::dir_off(i) + T::dir_lead(i), A[k][i]);
+                        // layout constants forced to compile-time values (evaluated at run time they would read the host-side
+                        // lattice table: the compiler then treats the path as unreachable and silently drops it)
+                        constexpr int so = T::dir_off(i) + T::dir_lead(i);
+                        pulled_from_row<CT, ST, VEC, L::E[i][0]>(rows + k * T::RB + so, A[k][i]);
                     });
             }
             __syncwarp();
@@ -360,7 +363,8 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
             // lane i < Q issues the bulk copies of direction i: source row (y - e_y, z - e_z) of its plane
             int ex_l = 0, ey_l = 0, ez_l = 0, off_l = 0;
             static_for<0, Q>([&](auto I) {
-                if (lane == I) { ex_l = L::E[I][0]; ey_l = L::E[I][1]; ez_l = L::E[I][2]; off_l = T::dir_off(I); }
+                constexpr int ex = L::E[I][0], ey = L::E[I][1], ez = L::E[I][2], so = T::dir_off(I);
+                if (lane == I) { ex_l = ex; ey_l = ey; ez_l = ez; off_l = so; }
             });
             const unsigned base_l = (unsigned)lane * plane + (unsigned)wrap_y(yw - ey_l) * sy;
             constexpr int NXD = []() { int n = 0; for (int i = 0; i < Q; ++i) n += L::E[i][0] != 0; return n; }();
@@ -420,7 +424,8 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                         static_for<0, Q>([&](auto I) {
                             constexpr int i = I;
                             CT f[VEC];
-                            pulled_from_row<CT, ST, VEC, L::E[i][0]>(land + k * T::RB + T::dir_off(i) + T::dir_lead(i) + xl, f);
+                            constexpr int so = T::dir_off(i) + T::dir_lead(i);
+                            pulled_from_row<CT, ST, VEC, L::E[i][0]>(land + k * T::RB + so + xl, f);
                             if constexpr (WREF) {
 #pragma unroll
                                 for (int v = 0; v < VEC; ++v) f[v] += p.wref[i];

@@ -1,6 +1,8 @@
 // lbm_launch.cuh -- host-side dispatch from run-time options to the kernel templates of lbm_core.cuh.
 // One translation unit per (lattice, compute dtype, storage dtype) instantiates launch<L,CT,ST>.
 #pragma once
+#include <cstdio>
+#include <cstdlib>
 #include "lbm_fused.cuh"
 #include "lbm_fused_ws.cuh"
 
@@ -23,6 +25,7 @@ struct LaunchArgs {
     int variant;         // OP_FUSED: 0 = default (warp-specialised k_fused_ws on D3Q19, lock-step k_fused_v on D2Q9);
                          //           -1 = lock-step kernel everywhere; 1.. = tuning experiments (LBM_FUSED_TUNING)
     int pfd;             // OP_FUSED (warp-specialised): L2 prefetch distance in planes
+    int* used_kernel;    // OP_FUSED, out: 1 = lock-step k_fused_v ran, 2 = warp-specialised k_fused_ws
     int wref;            // OP_FUSED: rho_ref != 0 (populations stored shifted by w_i rho_ref)
     cudaStream_t stream;
 };
@@ -175,6 +178,7 @@ cudaError_t launch(const LaunchArgs& a) {
                             g.y = (unsigned)((p.ny + a.i0 - 1) / a.i0);
                         }
                         k_fused_v<L, NC, CT, ST, C_, VEC, WX, TY, (PF != 0)><<<g, T::THREADS, 0, a.stream>>>(p, a.i0);
+                        if (a.used_kernel) *a.used_kernel = 2;  // LBM_PATH_ONE_PASS_LOCKSTEP
                         done = true;
                     };
                     constexpr FusedShape fs = fused_shape<L, CT, ST, NC>();
@@ -187,16 +191,23 @@ cudaError_t launch(const LaunchArgs& a) {
                             static int ready = 0;   // 0 unknown, 1 usable, -1 not usable
                             if (ready == 0) {
                                 cudaFuncAttributes fa;
-                                bool ok = cudaFuncGetAttributes(&fa, kern) == cudaSuccess &&
-                                          fa.numRegs * T::THREADS >= T::REG_PROD * T::NPW * 32 + T::REG_CONS * T::NCW * 32 &&
-                                          cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM) == cudaSuccess;
-                                ready = ok ? 1 : -1;
+                                const cudaError_t e1 = cudaFuncGetAttributes(&fa, kern);
+                                const bool regs_ok = e1 == cudaSuccess &&
+                                                     fa.numRegs * T::THREADS >= T::REG_PROD * T::NPW * 32 + T::REG_CONS * T::NCW * 32;
+                                const cudaError_t e2 = regs_ok ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                                                      (int)T::SMEM) : cudaErrorUnknown;
+                                ready = (regs_ok && e2 == cudaSuccess) ? 1 : -1;
+                                if (ready < 0 && std::getenv("LBM_VERBOSE"))
+                                    std::fprintf(stderr, "[lbm] k_fused_ws unusable: attr=%s regs=%d smem=%zu set=%s; lock-step kernel used\n",
+                                                 cudaGetErrorString(e1), e1 == cudaSuccess ? fa.numRegs : -1, (size_t)T::SMEM,
+                                                 cudaGetErrorString(e2));
                                 cudaGetLastError();
                             }
                             if (ready < 0) return;
                             dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + TY - 1) / TY),
                                    (unsigned)((p.nz + a.i0 - 1) / a.i0));
                             kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0, a.pfd);
+                            if (a.used_kernel) *a.used_kernel = 3;  // LBM_PATH_ONE_PASS_WS
                             done = true;
                         }
                     };

@@ -30,6 +30,12 @@ def run_three(wl, inp, steps, oracle_wl=None):
     l0 = g1.kernel_launches
     g1.step(steps)
     assert g1.kernel_launches - l0 == steps      # one launch per step: K2F ran, not K1 + K2
+    import os
+    # k_fused_ws: D3Q19 and rows that are whole 16-byte vectors of the storage dtype; else the lock-step kernel
+    sbytes = {"f16": 2, "f32": 4, "f64": 8}[wl.get("store_dtype", wl.get("compute_dtype", "f64"))]
+    ws = wl["lattice"] == "D3Q19" and wl["nx"] % (16 // sbytes) == 0 and os.environ.get("LBM_TUNE_FUSED_VARIANT") != "-1"
+    want = "one_pass_ws" if ws else "one_pass_lockstep"
+    assert g1.hot_path == want, g1.hot_path        # and the intended kernel, not a silent fallback
     g2.step(steps)
     return ([o.get_populations(k) for k in range(o.nc)], [g1.get_populations(k) for k in range(o.nc)],
             [g2.get_populations(k) for k in range(o.nc)], o)
@@ -61,6 +67,39 @@ def test_config5_fp32_100_steps(kernel, monkeypatch):
     assert_parity(f2, f1, fluid, 2e-6, relative=True)
 
 
+@pytest.mark.parametrize("dims,dtype,store", [((136, 26, 12), "f64", "f64"), ((264, 27, 10), "f32", "f32"),
+                                              ((272, 26, 9), "f32", "f16"), ((136, 34, 7), "f64", "f32")])
+def test_d3q19_several_tiles_all_dtypes(dims, dtype, store, monkeypatch):
+    """Domains several tiles wide and tall (tiles on and off the periodic seams, ragged last tiles), every dtype
+    combination the warp-specialised kernel is built for."""
+    monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "5")
+    wl, _ = W.config5(16, dtype, store_dtype=store)
+    wl.update(nx=dims[0], ny=dims[1], nz=dims[2])
+    inp = small_inputs(wl, 31, 0.05, 0.3)
+    steps = 30
+    fo, f1, f2, o = run_three(wl, inp, steps, oracle_wl=None if dtype == "f64" and store == "f64" else with_dtype(wl, "f64") if store != "f16" else None)
+    fluid = np.ones(o.N, bool)
+    if store == "f16":
+        assert_parity(fo, f1, fluid, TOL16, relative=True)      # oracle emulates the fp16 rounding at the store
+    elif dtype == "f64" and store == "f64":
+        assert_parity(fo, f1, fluid, TOL64, relative=False)
+        assert_parity(f2, f1, fluid, 1e-13, relative=False)
+    elif dtype == "f64":                                          # fp64 compute, fp32 storage
+        assert_parity(f2, f1, fluid, 1e-6, relative=True)
+    else:
+        assert_parity(fo, f1, fluid, TOL32, relative=True)
+
+
+def test_two_components_several_tiles_fp32():
+    g = 3.5 / 3.0
+    wl = dict(name="x", lattice="D3Q19", nx=140, ny=26, nz=7, n_components=2, periodic=(True, True, True),
+              psi_kind=["SC93", "SC93"], eos=[dict(rho0=1.0), dict(rho0=1.0)], G=[[0.0, g], [g, 0.0]],
+              collision="BGK", tau=[1.0, 1.0], forcing="EDM", compute_dtype="f32", store_dtype="f32")
+    inp = small_inputs(wl, 6, 0.4, 0.9)
+    fo, f1, f2, o = run_three(wl, inp, 30, oracle_wl=with_dtype(wl, "f64"))
+    assert_parity(fo, f1, np.ones(o.N, bool), TOL32, relative=True)
+
+
 def test_config5_fp16_storage():
     wl, inp = W.config5(32, "f32", store_dtype="f16")
     fo, f1, f2, o = run_three(wl, inp, 100)   # the oracle emulates the fp16 rounding at the store (R16)
@@ -86,7 +125,7 @@ def test_d2q9_fp64(nx, ny, monkeypatch):
     assert_parity(fo, f1, np.ones(o.N, bool), TOL64, relative=False)
 
 
-@pytest.mark.parametrize("lattice,n", [("D2Q9", (46, 23, 1)), ("D3Q19", (22, 10, 9))])
+@pytest.mark.parametrize("lattice,n", [("D2Q9", (46, 23, 1)), ("D3Q19", (24, 10, 9)), ("D3Q19", (22, 10, 9))])
 @pytest.mark.parametrize("collision", ["BGK", "MRT"])
 @pytest.mark.parametrize("forcing", ["EDM", "SHIFT"])
 def test_two_components_variants_fp32(lattice, n, collision, forcing):
