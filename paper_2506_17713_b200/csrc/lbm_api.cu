@@ -484,9 +484,8 @@ FusedShape fused_shape_of(const lbm_config_t& c, int variant) {
     auto pick = [&](auto L) -> FusedShape {
         using LT = decltype(L);
         const bool f32 = c.compute_dtype == LBM_F32;
-        if (variant == 12) {   // tuning: k_fused_ws with three stages of 6 rows
-            FusedShape d = c.compute_dtype == LBM_F32 ? fused_shape<LT, float, float, 1>() : fused_shape<LT, double, double, 1>();
-            if (LT::D == 3 && c.n_components == 1 && d.vec > 0) return FusedShape{d.vec, 1, 6};
+        if (variant == 13) {   // tuning: k_fused_ws with half-width tiles and four stages
+            if (LT::D == 3 && c.n_components == 1 && f32) return FusedShape{2, 1, 8};
             return none;
         }
         if (variant > 0) {

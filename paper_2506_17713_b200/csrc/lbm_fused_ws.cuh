@@ -104,7 +104,8 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, u
 template <class L, int NC, class CT, class ST, int VEC, int TY, int NSTG>
 struct WsTile {
     static_assert(L::D == 3, "the warp-specialised kernel marches along z");
-    static_assert(NSTG == 2 || NSTG == 3, "two or three stages");
+    static_assert(NSTG >= 2 && NSTG <= 4, "two to four stages");
+    static constexpr int AHEAD = NSTG - 2;                         // planes whose copies fly ahead of the one being summed
     static constexpr int Q = L::Q;
     static constexpr int ROWS = TY + 2;
     static constexpr int TX = 32 * VEC;
@@ -117,7 +118,7 @@ struct WsTile {
     static constexpr int dir_lead(int i) { return L::E[i][0] > 0 ? PADS : 0; }          // offset of the tile's first cell
     static constexpr int dir_off(int i) { int o = 0; for (int j = 0; j < i; ++j) o += dir_pitch(j); return o; }
     static constexpr int RB = dir_off(Q);                                                 // one component of a tile row
-    static constexpr int NS = 5;                                   // psi ring slots (>= 5, see the hand-over notes)
+    static constexpr int NS = NSTG + 3;                            // psi ring slots (>= NSTG + 2, see the hand-over notes)
     // warps come in warpgroups of four (setmaxnreg): consumer group = TY row consumers (+ the two ring warps if two
     // warps are spare there), producer group = ROWS row producers (+ the ring warps otherwise)
     static constexpr int NCONS = TY;                               // row consumers
@@ -130,7 +131,7 @@ struct WsTile {
     static constexpr size_t ROW_ELEMS = (size_t)NC * RB;                            // one tile row, all directions
     static constexpr size_t STAGE_ELEMS = ROW_ELEMS * TY;                           // one stage (interior rows)
     static constexpr size_t PSI_ELEMS = (size_t)NS * NC * ROWS * PITCH;
-    static constexpr size_t SMEM = sizeof(ST) * (NSTG * STAGE_ELEMS + 4 * ROW_ELEMS) + sizeof(CT) * PSI_ELEMS + 8 * (2 * NSTG + NS + 2 * ROWS);
+    static constexpr size_t SMEM = sizeof(ST) * (NSTG * STAGE_ELEMS + 2 * NSTG * ROW_ELEMS) + sizeof(CT) * PSI_ELEMS + 8 * (2 * NSTG + NS + NSTG * ROWS);
     // register split: the pool is THREADS x (registers at launch)
     static constexpr int REG_LAUNCH = (65536 / THREADS) / 8 * 8;
     static constexpr int REG_PROD = 56;
@@ -169,19 +170,19 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
     constexpr int Q = L::Q;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     ST* stage = reinterpret_cast<ST*>(smem_raw);                        // [NSTG][TY][NC][RB]
-    ST* halo = stage + NSTG * T::STAGE_ELEMS;                            // [2 planes][2 halo rows][NC][RB] landing rows
-    CT* psi_s = reinterpret_cast<CT*>(halo + 4 * T::ROW_ELEMS);         // [NS][NC][ROWS][PITCH]
+    ST* halo = stage + NSTG * T::STAGE_ELEMS;                            // [NSTG planes][2 halo rows][NC][RB] landing rows
+    CT* psi_s = reinterpret_cast<CT*>(halo + 2 * NSTG * T::ROW_ELEMS);         // [NS][NC][ROWS][PITCH]
     uint64_t* bars = reinterpret_cast<uint64_t*>(psi_s + T::PSI_ELEMS); // full[NSTG], empty[NSTG], psi_ready[NS]
     uint64_t* bar_full = bars;
     uint64_t* bar_empty = bars + NSTG;
     uint64_t* bar_psi = bars + 2 * NSTG;
-    uint64_t* bar_land = bar_psi + T::NS;                               // [2][ROWS] bulk copies of a row producer landed
+    uint64_t* bar_land = bar_psi + T::NS;                               // [NSTG][ROWS] bulk copies of a row producer landed
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTG; ++s) { mbar_init(bar_full + s, TY); mbar_init(bar_empty + s, T::NCONS); }
         for (int s = 0; s < T::NS; ++s) mbar_init(bar_psi + s, T::NPSI);
-        for (int s = 0; s < 2 * T::ROWS; ++s) mbar_init(bar_land + s, 1);
+        for (int s = 0; s < NSTG * T::ROWS; ++s) mbar_init(bar_land + s, 1);
     }
     __syncthreads();
 
@@ -373,14 +374,14 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
             // where plane pl of this row lands: interior rows in stage (it mod NSTG), halo rows in their own two buffers
             auto landing = [&](int it) -> ST* {
                 return interior ? stage + (size_t)((it + NSTG) % NSTG) * T::STAGE_ELEMS + (size_t)(r - 1) * T::ROW_ELEMS
-                                : halo + (size_t)(2 * ((it + 1) & 1) + (r == 0 ? 0 : 1)) * T::ROW_ELEMS;
+                                : halo + (size_t)(2 * ((it + NSTG) % NSTG) + (r == 0 ? 0 : 1)) * T::ROW_ELEMS;
             };
             // start the copies of plane pl (after its stage slot has been released by the consumers)
             auto issue = [&](int pl) {
                 const int it = pl - m0;
                 if (it >= 0) mbar_wait(bar_empty + it % NSTG, ((it / NSTG) & 1) ^ 1);
                 if (!used) return;
-                uint64_t* lb = bar_land + ((it + 1) & 1) * T::ROWS + r;
+                uint64_t* lb = bar_land + ((it + NSTG) % NSTG) * T::ROWS + r;
                 ST* land = landing(it);
                 if (lane == 0) mbar_expect_tx(lb, land_bytes);
                 __syncwarp();
@@ -404,18 +405,22 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                 }
             };
             WS_T0();
+            // With more than two stages the copies run AHEAD planes in front of the plane being summed, so that the
+            // memory system always has a plane in flight.  (With two stages that does not work: the slot of plane pl+1 is
+            // only released once the consumers have collided plane pl-2, and the producer would block in front of a rho
+            // pass whose data has already landed.)
+#pragma unroll
+            for (int d = 0; d < T::AHEAD; ++d)
+                if (m0 - 1 + d <= m1) issue(m0 - 1 + d);
             for (int pl = m0 - 1; pl <= m1; ++pl) {
                 const int it = pl - m0;                       // -1 .. mchunk
                 const bool staged = it >= 0 && pl < m1;       // planes m0-1 and m1 only feed psi
                 const int s = (it + NSTG) % NSTG;
-                // (Issuing the copies of plane pl+1 here as well, before summing plane pl, was tried and is slower with two
-                // stages: the slot of pl+1 is only released once the consumers have collided plane pl-2, so the producer
-                // blocks in front of a rho pass whose data has already landed.)
-                issue(pl);
+                if (pl + T::AHEAD <= m1) issue(pl + T::AHEAD);
                 WS_TICK(0);
                 const int q = it + 1, slot = q % T::NS;
                 const ST* land = landing(it);
-                if (used) mbar_wait(bar_land + ((it + 1) & 1) * T::ROWS + r, ((it + 1) >> 1) & 1);
+                if (used) mbar_wait(bar_land + s * T::ROWS + r, ((it + 1) / NSTG) & 1);
                 WS_TICK(1);
                 if (act) {
 #pragma unroll

@@ -220,14 +220,13 @@ cudaError_t launch(const LaunchArgs& a) {
                                 else go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<2>{}, IC<0>{}, IC<1>{});
                                 if (done) return;
                             }
-#ifdef LBM_FUSED_TUNING
-                            if constexpr (NC == 1) {
-                                if (a.variant == 12 && !a.wref) {
-                                    go_ws(IC<fs.vec>{}, IC<6>{}, IC<3>{}, IC<0>{}, IC<1>{});
+                            // variant 13: half-width tiles (VEC / 2) and four stages, the copies two planes ahead
+                            if constexpr (NC == 1 && sizeof(CT) == 4) {
+                                if (a.variant == 13 && !a.wref) {
+                                    go_ws(IC<fs.vec / 2>{}, IC<8>{}, IC<4>{}, IC<0>{}, IC<1>{});
                                     if (done) return;
                                 }
                             }
-#endif
                         }
                         go(IC<fs.vec>{}, IC<fs.wx>{}, IC<fs.ty>{}, IC<1>{});
                     }
