@@ -261,7 +261,7 @@ def gpu_run(torch, workload: str, steps: int, warmup: int, dist, want_roofline=T
 def reduce_max(torch, dist, x: float) -> float:
     if dist is None:
         return x
-    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    t = torch.tensor([x], dtype=torch.float64, device="cuda" if torch.cuda.is_available() else "cpu")
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
 

@@ -11,17 +11,19 @@
 //
 //   producers (one warp per tile row incl. the two halo rows, VEC cells per lane, + two warps for the ring columns)
 //       plane p: copy the row segments the pull needs (S7 read side: 19 source rows, one per direction, each with one
-//       vector of padding where the pull is shifted in x) from global memory straight into a 2-deep stage in shared
-//       memory with cp.async (LDGSTS): the whole plane-row is in flight at once and costs no registers.  Then sum
-//       rho from the stage, evaluate psi -> psi ring in shared memory (5 planes).
+//       16-byte vector of padding on the side the pull is shifted to in x) from global memory straight into a stage in
+//       shared memory with bulk asynchronous copies (cp.async.bulk, SASS UBLKCP; lane i issues direction i; completion
+//       on a per-row mbarrier): the whole plane-row is in flight at once and costs no registers.  Then sum rho from
+//       the stage, evaluate psi -> psi ring in shared memory.
 //   consumers (one warp per interior row)
 //       plane m: take the pulled populations from the stage into registers, release the stage, wait for psi of
 //       plane m+1, then moments, force from the psi planes m-1, m, m+1, collision, store (S7 write side).
 //
 //   Hand-over is by mbarriers in shared memory (full / empty per stage, one "psi ready" barrier per ring slot).
 //   Producers need few registers, consumers hold Q x VEC values: the register file is re-split with setmaxnreg
-//   after the role dispatch.  A first version loaded through registers: ptxas split the 29 loads of a plane-row into
-//   ~12 batches and the producers paid the memory latency once per batch (profiles/): hence the asynchronous copies.
+//   after the role dispatch.  Earlier versions, measured on 512^3: loads through registers (ptxas split
+//   the 29 loads of a plane-row into ~12 batches under the producers' register cap, one memory latency per batch),
+//   then per-lane cp.async (LSU-bound issue), then these bulk copies.
 //   Addresses are 32-bit element offsets scaled onto per-thread 64-bit bases (mad.wide.u32): two instructions per
 //   access instead of five.
 // Arithmetic (order of every sum) is that of K1 / K2 in lbm_hot.cuh.
@@ -74,21 +76,6 @@ __device__ __forceinline__ T* at_u32(T* base, unsigned idx) {
     return r;
 }
 
-// asynchronous global -> shared copy of BYTES (4, 8 or 16) per thread
-template <int BYTES>
-__device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
-    if constexpr (BYTES == 16)
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
-    else
-        asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "n"(BYTES) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() {
-    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
-}
-
-// TY interior rows per tile, NSTG stages.  With two stages producer and consumer are still coupled (the consumer of
-// plane m needs psi of plane m+1, whose producer could only start when the stage of plane m-1 was released): the step
-// period is the mean of their times, not the maximum; a third stage decouples them.
 // bulk asynchronous copy (TMA unit, SASS UBLKCP): `bytes` contiguous bytes global -> shared, 16-byte aligned on both
 // sides, completion counted on an mbarrier (complete_tx)
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
@@ -101,6 +88,9 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, u
                  : "memory");
 }
 
+// TY interior rows per tile, NSTG stages.  With two stages producer and consumer stay coupled (the consumer of plane m
+// needs psi of plane m+1, whose copies could only start when the slot of plane m-1 was released): the step period is
+// about the mean of their times, not the maximum.  More stages let the copies run AHEAD, but only fit smaller tiles.
 template <class L, int NC, class CT, class ST, int VEC, int TY, int NSTG>
 struct WsTile {
     static_assert(L::D == 3, "the warp-specialised kernel marches along z");
