@@ -22,6 +22,9 @@
 //   conservation (halfway bounce-back).
 //   viscosity nu = c_s^2 (tau - 1/2) from shear-wave decay, Poiseuille flow
 //   between pressure faces (first-order pin of the anti-bounce-back faces).
+//   A-weighted Zhang-Chen force (Eq. 11-13): F_ZC = -grad U against
+//   a re-typed EOS, weighted sum, coexistence -> Maxwell with A ~ -0.19,
+//   mass / momentum conservation.
 //   PARITY UNPINNED: the O(u^2) terms of the pressure-face (anti-bounce-back)
 //   formula -- reading R10 -- have no paper value or closed form to be held to;
 //   see DESIGN.md.
@@ -94,6 +97,7 @@ struct olbm_config {
     double tau[2];             // BGK tau; for MRT = 1/s_nu (used in S5 and shift forcing)
     double mrt_rates[2][19];   // diagonal of S, moment order of R9
     double rho_ref;            // storage shift: stored = f_i - w_i*rho_ref (R16)
+    double zc_A[2];            // A_kk of Eq. 11/13: F^k = A_kk F_ZC^k + (1 - A_kk) F_SC^k; 0 = pure Shan-Chen
 };
 }
 
@@ -228,7 +232,7 @@ struct Sim : SimBase {
     int face_kind[6];
     double face_rho[6][2];
     double face_u[6][3];
-    std::vector<T> f[2], fstar[2], rho[2], psi[2], j[2][3], F[2][3];
+    std::vector<T> f[2], fstar[2], rho[2], psi[2], U[2], j[2][3], F[2][3];
     std::vector<T> ucom[3];  // common velocity u' of S5
     int64_t steps_done = 0;
 
@@ -257,6 +261,7 @@ struct Sim : SimBase {
             fstar[k].assign((size_t)q * N, T(0));
             rho[k].assign(N, T(0));
             psi[k].assign(N, T(0));
+            U[k].assign(N, T(0));
             for (int a = 0; a < 3; ++a) { j[k][a].assign(N, T(0)); F[k][a].assign(N, T(0)); }
         }
         for (int a = 0; a < 3; ++a) ucom[a].assign(N, T(0));
@@ -430,6 +435,16 @@ struct Sim : SimBase {
         return rad > T(0) ? std::sqrt(rad) : T(0);
     }
 
+    // Eq. 12, second line: U^k = alpha^k p_EOS^k - c_s^2 rho^k (EOS kinds only; the Zhang-Chen term needs an EOS)
+    T zc_potential(int k, T r) const {
+        int kind = c.psi_kind[k];
+        if (kind > PSI_EOS_RKS) return T(0);
+        T Tc = (T)eos_critical_temperature(kind, c.eos_a[k], c.eos_b[k], c.eos_R[k]);
+        T p = eos_pressure<T>(kind, (T)c.eos_a[k], (T)c.eos_b[k], (T)c.eos_R[k], (T)c.eos_omega[k],
+                              (T)c.eos_T[k], Tc, r);
+        return (T)c.alpha[k] * p - cs2 * r;
+    }
+
     // S1..S4: moments, virtual density, psi, force -- everything S6 needs.
     void compute_fields() {
         const int nc = c.n_components;
@@ -477,6 +492,11 @@ struct Sim : SimBase {
             for (int64_t id = 0; id < N; ++id)
                 if (!solid[id]) psi[k][id] = pseudopotential(k, rho[k][id]);
             for (size_t b = 0; b < bsolid.size(); ++b) psi[k][bsolid[b]] = pseudopotential(k, rho[k][bsolid[b]]);
+            if (c.zc_A[k] != 0.0) {
+                for (int64_t id = 0; id < N; ++id)
+                    if (!solid[id]) U[k][id] = zc_potential(k, rho[k][id]);
+                for (size_t b = 0; b < bsolid.size(); ++b) U[k][bsolid[b]] = zc_potential(k, rho[k][bsolid[b]]);
+            }
         }
         // S4 (Eq. 13 F_SC; wetting folded in through psi(rho_s)):
         // F^k(x) = -psi^k(x) sum_k' g_kk' sum_i G_i psi^k'(x+e_i) e_i,  G_i = w_i/c_s^2 (R2)
@@ -496,6 +516,16 @@ struct Sim : SimBase {
                     for (int a = 0; a < d; ++a) acc[a] += (T)c.G[k][kp] * s[a];
                 }
                 for (int a = 0; a < 3; ++a) F[k][a][id] = -psi[k][id] * acc[a];
+                // Eq. 13: F^k = A_kk F_ZC^k + (1 - A_kk) F_SC^k,  F_ZC^k = -sum_i G_i U^k(x+e_i) e_i
+                if (c.zc_A[k] != 0.0) {
+                    T z[3] = {T(0), T(0), T(0)};
+                    for (int i = 1; i < q; ++i) {
+                        T v = gw[i] * U[k][scalar_nbr(xyz, i)];
+                        for (int a = 0; a < d; ++a) z[a] += v * (T)e[i][a];
+                    }
+                    const T A = (T)c.zc_A[k];
+                    for (int a = 0; a < 3; ++a) F[k][a][id] = A * (-z[a]) + (T(1) - A) * F[k][a][id];
+                }
             }
         }
         // S5 (R6): common velocity u' = sum_k (j^k/tau_k) / sum_k (rho^k/tau_k); = j/rho for one component

@@ -52,6 +52,7 @@ class _Config(C.Structure):
         ("tau", C.c_double * 2),
         ("mrt_rates", (C.c_double * 19) * 2),
         ("rho_ref", C.c_double),
+        ("zc_A", C.c_double * 2),
     ]
 
 
@@ -147,6 +148,7 @@ def make_config(wl: dict) -> _Config:
             c.mrt_rates[k][r] = float(rates[k][r]) if rates is not None else 1.0 / c.tau[k]
         for kp in range(nc):
             c.G[k][kp] = float(G[k][kp])
+        c.zc_A[k] = float(wl.get("zc_A", [0.0] * nc)[k])
     return c
 
 

@@ -165,3 +165,55 @@ def test_contact_angle_neutral_and_monotone():
     dx2, t2 = _meniscus_offset(0.30)
     assert 0 < dx1 < dx2
     assert angle > t1 > t2 > 30.0
+
+
+# ------------------------------------------------------------------ NEXT-1: A-weighted Zhang-Chen force (Eq. 11-13)
+def _cs_wl(n, A, lattice="D2Q9", **kw):
+    return base_wl(lattice, n, psi_kind=["CS"], eos=[dict(a=W.CS_A, b=W.CS_B, R=W.CS_R, T=W.CS_T_085)], G=[[-1.0]],
+                   zc_A=[A], **kw)
+
+
+@pytest.mark.parametrize("lattice,n", [("D2Q9", (64, 48, 1)), ("D3Q19", (40, 32, 24))])
+def test_zhang_chen_force_is_minus_grad_U(lattice, n):
+    """A = 1: F = F_ZC = -sum_i G_i U(x+e_i) e_i is a second-order approximation of -grad U with
+    U = alpha p_EOS - c_s^2 rho (Eq. 11 first term, Eq. 12 second line); the EOS pressure is re-typed here."""
+    d = 2 if lattice == "D2Q9" else 3
+    z, y, x = np.meshgrid(np.arange(n[2]), np.arange(n[1]), np.arange(n[0]), indexing="ij")
+    kx, ky = 2 * np.pi / n[0], 2 * np.pi / n[1]
+    rho = 0.15 + 0.05 * np.sin(kx * x) * np.cos(ky * y)
+    drx, dry = 0.05 * kx * np.cos(kx * x) * np.cos(ky * y), -0.05 * ky * np.sin(kx * x) * np.sin(ky * y)
+    a, b, RT = W.CS_A, W.CS_B, W.CS_R * W.CS_T_085
+    eta = lambda r: b * r / 4
+    p = lambda r: r * RT * (1 + eta(r) + eta(r) ** 2 - eta(r) ** 3) / (1 - eta(r)) ** 3 - a * r * r
+    h = 1e-6
+    dU = ((p(rho + h) - p(rho - h)) / (2 * h) - 1.0 / 3.0)        # dU/drho
+    s = make_oracle(_cs_wl(n, 1.0, lattice), dict(rho=[rho.reshape(-1)]))
+    F = s.get_force(0)
+    scale = np.abs(dU * drx).max()
+    assert np.abs(F[0] + (dU * drx).reshape(-1)).max() < 0.03 * scale
+    assert np.abs(F[1] + (dU * dry).reshape(-1)).max() < 0.03 * scale
+    if d == 3:
+        assert np.abs(F[2]).max() < 1e-15
+    # A = 0 is the plain Shan-Chen force, A = 0.3 the weighted sum of the two (Eq. 13, first line)
+    f0 = make_oracle(_cs_wl(n, 0.0, lattice), dict(rho=[rho.reshape(-1)])).get_force(0)
+    f3 = make_oracle(_cs_wl(n, 0.3, lattice), dict(rho=[rho.reshape(-1)])).get_force(0)
+    assert np.abs(f3 - (0.3 * F + 0.7 * f0)).max() < 1e-15
+    # both forms discretise the same continuum force: -grad U = -g psi grad psi since U = g psi^2 / 2
+    assert np.abs(F[0] - f0[0]).max() < 0.05 * scale
+
+
+def test_zhang_chen_weight_brings_coexistence_to_maxwell_and_conserves():
+    """the weighted force reaches densities the single schemes do not.  For CS at T_r = 0.85 a
+    weight A ~ -0.19 brings the flat-interface vapour density from -8 % (A = 0, test above) to within 1.5 % of Maxwell's
+    construction and keeps the liquid within 0.2 %.  Mass is conserved to rounding and total momentum stays zero
+    (F_ZC sums to zero over a periodic box just as F_SC does)."""
+    nx, ny = 128, 2
+    s = make_oracle(_cs_wl((nx, ny, 1), -0.19), dict(rho=[_flat(nx, ny, W.CS_RHO_L_085, W.CS_RHO_V_085)]))
+    m0 = s.get_macroscopic()[0][0].sum()
+    s.step(8000)
+    rho, u, p = s.get_macroscopic()
+    r = rho[0].reshape(ny, nx)[0]
+    assert abs(r[nx // 2] / W.CS_RHO_L_085 - 1) < 2e-3
+    assert abs(r[0] / W.CS_RHO_V_085 - 1) < 1.5e-2
+    assert abs(rho[0].sum() / m0 - 1) < 1e-12
+    assert np.abs(s.get_force(0).sum(axis=1)).max() < 1e-12
