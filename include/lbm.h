@@ -123,6 +123,9 @@ typedef struct {
     double tau[2];           /* BGK relaxation time; with MRT = 1/s_nu (enters the common velocity and LBM_SHIFT) */
     double mrt_rates[2][19]; /* diagonal of S in the moment order of DESIGN.md R9 (first q entries used) */
     double rho_ref;          /* populations are stored as f_i - w_i*rho_ref (reading R16); 0 = plain */
+    double zc_A[2];          /* A_kk of Eq. 11 / 13: F^k = A_kk F_ZC^k + (1 - A_kk) F_SC^k with the Zhang-Chen
+                                force F_ZC^k = -sum_i G_i U^k(x+e_i) e_i, U^k = alpha p_EOS - c_s^2 rho (Eq. 12).  0 = plain
+                                Shan-Chen.  Non-zero needs an EOS psi kind (LBM_E_INVALID otherwise) and runs the two-pass path. */
 } lbm_config_t;
 
 /* Bytes of device workspace lbm_create needs for cfg; 0 if cfg is invalid. */

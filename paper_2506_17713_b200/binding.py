@@ -49,7 +49,7 @@ class lbm_config_t(C.Structure):
         ("collision", C.c_int32), ("forcing", C.c_int32), ("compute_dtype", C.c_int32), ("store_dtype", C.c_int32),
         ("flags", C.c_uint32), ("pad_", C.c_int32),
         ("eos", lbm_eos_t * 2), ("G", (C.c_double * 2) * 2), ("wet", lbm_wetting_t * 2),
-        ("tau", C.c_double * 2), ("mrt_rates", (C.c_double * 19) * 2), ("rho_ref", C.c_double),
+        ("tau", C.c_double * 2), ("mrt_rates", (C.c_double * 19) * 2), ("rho_ref", C.c_double), ("zc_A", C.c_double * 2),
     ]
 
 
@@ -149,6 +149,7 @@ def make_config(wl: dict) -> lbm_config_t:
             c.mrt_rates[k][r] = float(rates[k][r]) if rates is not None else 1.0 / c.tau[k]
         for kp in range(nc):
             c.G[k][kp] = float(G[k][kp])
+        c.zc_A[k] = float(wl.get("zc_A", [0.0] * nc)[k])
     return c
 
 

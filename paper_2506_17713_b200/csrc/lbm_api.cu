@@ -90,6 +90,7 @@ int check_config(const lbm_config_t* c) {
             if (!(e.b > 0.0) || !(e.R > 0.0) || !(e.T > 0.0)) return LBM_E_INVALID;
         }
         if (e.psi_kind == LBM_PSI_SC93 && !(e.rho0 > 0.0)) return LBM_E_INVALID;
+        if (c->zc_A[k] != 0.0 && e.psi_kind > LBM_PSI_EOS_RKS) return LBM_E_INVALID;   // U of Eq. 12 needs an EOS
         if (!(c->tau[k] > 0.5)) return LBM_E_INVALID;
     }
     return LBM_OK;
@@ -221,6 +222,9 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
             aalpha = e.a * s * s;
         }
         p.eos_aalpha[k] = (CT)aalpha;
+        p.zc[k] = c.zc_A[k] != 0.0 ? 1 : 0;
+        p.zcA[k] = (CT)c.zc_A[k];
+        p.zc_hg[k] = (CT)(0.5 * c.G[k][k]);
         p.wet_phi[k] = (CT)c.wet[k].phi;
         p.wet_drho[k] = (CT)c.wet[k].drho;
         p.wet_lo[k] = (CT)c.wet[k].lo;
@@ -343,6 +347,13 @@ __global__ void k_export_flags(int N, const uint32_t* __restrict__ in, uint32_t*
     if (id < N) out[id] = in[id] & (SOLID_BIT | LINK_MASK);
 }
 
+// psi export of a component with a Zhang-Chen weight: the field holds the signed root, psi is its positive part
+template <class CT>
+__global__ void k_clamp0(CT* __restrict__ x, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n && x[i] < CT(0)) x[i] = CT(0);
+}
+
 template <class TI, class TO>
 __global__ void k_convert(const TI* __restrict__ in, TO* __restrict__ out, long long n) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -435,7 +446,9 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.coll = (h->cfg.flags & LBM_FLAG_NO_COLLIDE) ? 2 : (h->cfg.collision == LBM_MRT ? 1 : 0);
     a.bnd = h->bnd ? 1 : 0;
     a.vec = h->vec;
-    a.list = (h->use_list && (op == OP_MOMENTS || op == OP_STEP)) ? 1 : 0;
+    const bool zc = h->cfg.zc_A[0] != 0.0 || (h->cfg.n_components > 1 && h->cfg.zc_A[1] != 0.0);
+    a.zc = (zc && op == OP_STEP && !(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) ? 1 : 0;
+    a.list = (h->use_list && (op == OP_MOMENTS || (op == OP_STEP && !a.zc))) ? 1 : 0;
     a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
     a.variant = h->fvariant;
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;
@@ -506,6 +519,7 @@ void plan_fused(lbm* h) {
     h->use_fused = false;
     const lbm_config_t& c = h->cfg;
     if (c.flags & (LBM_FLAG_TWO_PASS | LBM_FLAG_NO_COLLIDE)) return;
+    if (c.zc_A[0] != 0.0 || (c.n_components > 1 && c.zc_A[1] != 0.0)) return;   // Zhang-Chen weight: two-pass path
     if (h->bnd || h->fshape.vec == 0 || c.nx % h->fshape.vec != 0) return;
     if ((unsigned long long)c.n_components * h->q * (unsigned long long)h->plane >= (1ULL << 32)) return;   // 32-bit element offsets
     if (h->d == 3 && c.nx % (16 / (int)h->sbytes) != 0 && h->fvariant == 0) h->fvariant = -1;   // k_fused_ws copies 16-byte pads
@@ -972,6 +986,14 @@ int lbm_get_psi(lbm_t* h, int comp, void* psi, int dtype, int on_device) {
     if (rc) return rc;
     if ((rc = do_launch(h, OP_MOMENTS))) return rc;
     if (h->nbsolid > 0 && (rc = do_launch(h, OP_VIRTUAL))) return rc;
+    if (h->cfg.zc_A[comp] != 0.0) {   // the next lbm_step recomputes the field anyway
+        char* field = h->ws + h->cv.psi + (size_t)comp * h->N * h->cbytes;
+        const unsigned grid = (unsigned)((h->N + 255) / 256);
+        if (h->cfg.compute_dtype == LBM_F32) k_clamp0<float><<<grid, 256, 0, h->stream>>>(reinterpret_cast<float*>(field), h->N);
+        else k_clamp0<double><<<grid, 256, 0, h->stream>>>(reinterpret_cast<double*>(field), h->N);
+        CU(cudaGetLastError());
+        h->launches++;
+    }
     const size_t eb = dtype_bytes(dtype);
     const int chunk = std::min(h->N, CHUNK_CELLS);
     const char* dev = h->ws + h->cv.psi + (size_t)comp * h->N * h->cbytes;

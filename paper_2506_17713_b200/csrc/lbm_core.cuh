@@ -148,6 +148,11 @@ struct KParams {
     int psi_kind[2];
     CT eos_a[2], eos_b[2], eos_RT[2], eos_aalpha[2], eos_sqrtT[2], eos_alpha[2], eos_rho0[2], eos_inv_gkk2[2];
     CT wet_phi[2], wet_drho[2], wet_lo[2], wet_hi[2];
+    // Zhang-Chen term (Eq. 11-13): zc[k] != 0 <=> A_kk != 0.  The psi field of such a component holds the SIGNED root
+    // s = sign(r) sqrt(|r|), r = 2 (alpha p - cs2 rho) / g_kk, so that both psi = max(s, 0) (Eq. 12, clamp R4) and
+    // U = alpha p - cs2 rho = (g_kk / 2) s |s| are available to the force without a second field.
+    int zc[2];
+    CT zcA[2], zc_hg[2];   // A_kk and g_kk / 2
     int face_kind[6];
     CT face_rho[6][2];
     CT face_u[6][3];
@@ -271,6 +276,7 @@ __device__ __forceinline__ CT psi_of_rho(const KParams<CT>& p, int k, CT r) {
     }
     // Eq. 12: psi = sqrt(2 (alpha p - cs2 rho) / g_kk), radicand clamped at 0 (R4); eos_inv_gkk2 = 2 / g_kk
     const CT rad = (p.eos_alpha[k] * pe - r * CT(1.0 / 3.0)) * p.eos_inv_gkk2[k];
+    if (p.zc[k]) return rad > CT(0) ? sqrt(rad) : -sqrt(-rad);   // signed root (see KParams::zc)
     return rad > CT(0) ? sqrt(rad) : CT(0);
 }
 
@@ -320,24 +326,37 @@ __global__ void __launch_bounds__(128) k_virtual_density(const __grid_constant__
 }
 
 // ------------------------------------------------------------------ shared pieces of K2 / export
-// S4: S[kp][a] = sum_i (w_i/cs2) psi^kp(x+e_i) e_ia
+// S4: S[kp][a] = sum_i (w_i/cs2) psi^kp(x+e_i) e_ia and, for components with a Zhang-Chen weight,
+// Z[kp][a] = sum_i (w_i/cs2) U^kp(x+e_i) e_ia (psi field = signed root there, see KParams::zc)
 template <class L, int NC, class CT>
-__device__ __forceinline__ void psi_gradient_sums(const KParams<CT>& p, const Cell& c, CT (&S)[NC][3]) {
+__device__ __forceinline__ void psi_gradient_sums(const KParams<CT>& p, const Cell& c, CT (&S)[NC][3], CT (&Z)[NC][3]) {
 #pragma unroll
     for (int kp = 0; kp < NC; ++kp) {
         S[kp][0] = S[kp][1] = S[kp][2] = CT(0);
+        Z[kp][0] = Z[kp][1] = Z[kp][2] = CT(0);
         const CT* ps = p.psi + (long long)kp * p.N + c.id;
+        const bool zc = p.zc[kp] != 0;
         static_for<1, L::Q>([&](auto I) {
             constexpr int i = I;
             constexpr int ex = L::E[i][0], ey = L::E[i][1], ez = L::E[i][2];
             constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
-            const CT v = gw * __ldg(ps + nbr_offset<ex, ey, ez>(c));
+            const CT s = __ldg(ps + nbr_offset<ex, ey, ez>(c));
+            const CT v = gw * (zc && s < CT(0) ? CT(0) : s);
             if constexpr (ex == 1) S[kp][0] += v;
             if constexpr (ex == -1) S[kp][0] -= v;
             if constexpr (ey == 1) S[kp][1] += v;
             if constexpr (ey == -1) S[kp][1] -= v;
             if constexpr (ez == 1) S[kp][2] += v;
             if constexpr (ez == -1) S[kp][2] -= v;
+            if (zc) {
+                const CT u = gw * (p.zc_hg[kp] * s * fabs(s));
+                if constexpr (ex == 1) Z[kp][0] += u;
+                if constexpr (ex == -1) Z[kp][0] -= u;
+                if constexpr (ey == 1) Z[kp][1] += u;
+                if constexpr (ey == -1) Z[kp][1] -= u;
+                if constexpr (ez == 1) Z[kp][2] += u;
+                if constexpr (ez == -1) Z[kp][2] -= u;
+            }
         });
     }
 }
@@ -465,11 +484,15 @@ __global__ void __launch_bounds__(128) k_export_macro(const __grid_constant__ KP
         });
         rho[k] = r; j[k][0] = jx; j[k][1] = jy; j[k][2] = jz;
     }
-    CT S[NC][3];
-    psi_gradient_sums<L, NC, CT>(p, c, S);
+    CT S[NC][3], Z[NC][3];
+    psi_gradient_sums<L, NC, CT>(p, c, S, Z);
     CT psi[NC], rt = CT(0);
 #pragma unroll
-    for (int k = 0; k < NC; ++k) { psi[k] = p.psi[(long long)k * p.N + id]; rt += rho[k]; }
+    for (int k = 0; k < NC; ++k) {
+        psi[k] = p.psi[(long long)k * p.N + id];
+        if (p.zc[k] && psi[k] < CT(0)) psi[k] = CT(0);
+        rt += rho[k];
+    }
     if (u_out) {
 #pragma unroll
         for (int a = 0; a < L::D; ++a) {
@@ -480,7 +503,7 @@ __global__ void __launch_bounds__(128) k_export_macro(const __grid_constant__ KP
 #pragma unroll
                 for (int kp = 0; kp < NC; ++kp) acc += p.G[k][kp] * S[kp][a];
                 js += j[k][a];
-                Fs += -psi[k] * acc;
+                Fs += p.zc[k] ? (CT(1) - p.zcA[k]) * (-psi[k] * acc) - p.zcA[k] * Z[k][a] : -psi[k] * acc;
             }
             u_out[(long long)a * p.N + id] = (js + Fs * CT(0.5)) / rt;
         }

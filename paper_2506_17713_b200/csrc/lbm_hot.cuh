@@ -353,12 +353,41 @@ constexpr int dir_of(int dx, int dy, int dz) {
 // S4 sums for VEC cells: S[a][v] = sum_i (w_i/cs2) psi(x_v + e_i) e_ia  and psi at the cells themselves.
 // rowfn(IC<dy>, IC<dz>, IC<need_x>, t, left, right) delivers psi of the row (y+dy, z+dz): t[v] at the thread's VEC
 // cells and, when need_x, the values left of lane 0 / right of lane VEC-1 (global memory in K2, shared memory in K2F).
-template <class L, class CT, int VEC, class RowFn>
-__device__ __forceinline__ void psi_sums_rows(RowFn&& rowfn, CT (&S)[3][VEC], CT (&pc)[VEC]) {
+// ZC (Zhang-Chen weight, KParams::zc): the rows hold the signed root s; the sums use psi = max(s, 0) and
+// Zs[a][v] = sum_i (w_i/cs2) U(x_v + e_i) e_ia with U = hg s |s| is accumulated as well.
+template <class L, class CT, int VEC, bool ZC = false, class RowFn>
+__device__ __forceinline__ void psi_sums_rows(RowFn&& rowfn, CT (&S)[3][VEC], CT (&pc)[VEC], CT (*Zs)[VEC] = nullptr, CT hg = CT(0)) {
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int v = 0; v < VEC; ++v) S[a][v] = CT(0);
+        for (int v = 0; v < VEC; ++v) {
+            S[a][v] = CT(0);
+            if constexpr (ZC) Zs[a][v] = CT(0);
+        }
+    auto accumulate = [&](auto DY, auto DZ, auto HAS0, auto HASX, const CT (&t)[VEC], CT left, CT right, CT (*acc)[VEC]) {
+        constexpr int dy = DY, dz = DZ;
+        if constexpr (HAS0 != 0) {
+            constexpr int i = dir_of<L>(0, dy, dz);
+            constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                if constexpr (dy != 0) acc[1][v] += CT(gw * dy) * t[v];
+                if constexpr (dz != 0) acc[2][v] += CT(gw * dz) * t[v];
+            }
+        }
+        if constexpr (HASX != 0) {
+            constexpr int i = dir_of<L>(1, dy, dz);
+            constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                const CT m = v > 0 ? t[v - 1] : left;
+                const CT q = v < VEC - 1 ? t[v + 1] : right;
+                acc[0][v] += gw * (q - m);
+                if constexpr (dy != 0) acc[1][v] += CT(gw * dy) * (q + m);
+                if constexpr (dz != 0) acc[2][v] += CT(gw * dz) * (q + m);
+            }
+        }
+    };
     static_for<0, 9>([&](auto RW) {
         constexpr int dy = RW % 3 - 1, dz = RW / 3 - 1;
         constexpr bool centre = dy == 0 && dz == 0;
@@ -366,52 +395,44 @@ __device__ __forceinline__ void psi_sums_rows(RowFn&& rowfn, CT (&S)[3][VEC], CT
         if constexpr ((has0 || hasx || centre) && (L::D == 3 || dz == 0)) {
             CT t[VEC], left = CT(0), right = CT(0);
             rowfn(IC<dy>{}, IC<dz>{}, IC<(hasx ? 1 : 0)>{}, t, left, right);
+            if constexpr (ZC) {
+                CT u[VEC];
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) { u[v] = hg * t[v] * fabs(t[v]); t[v] = t[v] > CT(0) ? t[v] : CT(0); }
+                const CT ul = hg * left * fabs(left), ur = hg * right * fabs(right);
+                left = left > CT(0) ? left : CT(0);
+                right = right > CT(0) ? right : CT(0);
+                accumulate(IC<dy>{}, IC<dz>{}, IC<(has0 ? 1 : 0)>{}, IC<(hasx ? 1 : 0)>{}, u, ul, ur, Zs);
+            }
             if constexpr (centre) {
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) pc[v] = t[v];
             }
-            if constexpr (has0) {
-                constexpr int i = dir_of<L>(0, dy, dz);
-                constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
-#pragma unroll
-                for (int v = 0; v < VEC; ++v) {
-                    if constexpr (dy != 0) S[1][v] += CT(gw * dy) * t[v];
-                    if constexpr (dz != 0) S[2][v] += CT(gw * dz) * t[v];
-                }
-            }
-            if constexpr (hasx) {
-                constexpr int i = dir_of<L>(1, dy, dz);
-                constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
-#pragma unroll
-                for (int v = 0; v < VEC; ++v) {
-                    const CT m = v > 0 ? t[v - 1] : left;
-                    const CT q = v < VEC - 1 ? t[v + 1] : right;
-                    S[0][v] += gw * (q - m);
-                    if constexpr (dy != 0) S[1][v] += CT(gw * dy) * (q + m);
-                    if constexpr (dz != 0) S[2][v] += CT(gw * dz) * (q + m);
-                }
-            }
+            accumulate(IC<dy>{}, IC<dz>{}, IC<(has0 ? 1 : 0)>{}, IC<(hasx ? 1 : 0)>{}, t, left, right, S);
         }
     });
 }
 
 // psi rows from the global psi field (two-pass path)
-template <class L, class CT, int VEC>
-__device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VCell& c, CT (&S)[3][VEC], CT (&pc)[VEC]) {
-    psi_sums_rows<L, CT, VEC>(
+template <class L, class CT, int VEC, bool ZC = false>
+__device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VCell& c, CT (&S)[3][VEC], CT (&pc)[VEC],
+                                             CT (*Zs)[VEC] = nullptr, CT hg = CT(0)) {
+    psi_sums_rows<L, CT, VEC, ZC>(
         [&](auto DY, auto DZ, auto NX, CT (&t)[VEC], CT& left, CT& right) {
             const CT* row = ps + (c.zo[1 + DZ] + c.yo[1 + DY]);
             ld_vec<CT, CT, VEC>(row + c.x0, t);
             if constexpr (NX != 0) { left = __ldg(row + c.xm); right = __ldg(row + c.xp); }
         },
-        S, pc);
+        S, pc, Zs, hg);
 }
 
 // S4 + S5 for one cell: du^k = F^k / rho^k with F^k = -psi^k sum_k' g_kk' S^k' (Eq. 13, Eq. 5) and the common
 // velocity u' (R6) from the moments.
+// With a Zhang-Chen weight (Z != nullptr): F^k = (1 - A_kk) F_SC^k + A_kk F_ZC^k, F_ZC^k = -Z^k (Eq. 13).
 template <int NC, class CT>
 __device__ __forceinline__ void force_and_velocity(const KParams<CT>& p, const CT (&rho)[NC], const CT (&j)[NC][3],
-                                                   const CT (&S)[NC][3], const CT (&pc)[NC], CT (&u)[3], CT (&du)[NC][3]) {
+                                                   const CT (&S)[NC][3], const CT (&pc)[NC], CT (&u)[3], CT (&du)[NC][3],
+                                                   const CT (*Z)[3] = nullptr) {
     CT inv_r[NC];
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
@@ -421,7 +442,9 @@ __device__ __forceinline__ void force_and_velocity(const KParams<CT>& p, const C
             CT acc = CT(0);
 #pragma unroll
             for (int kp = 0; kp < NC; ++kp) acc += p.G[k][kp] * S[kp][a];
-            du[k][a] = (-pc[k] * acc) * inv_r[k];
+            CT F = -pc[k] * acc;
+            if (Z != nullptr && p.zc[k]) F = (CT(1) - p.zcA[k]) * F - p.zcA[k] * Z[k][a];
+            du[k][a] = F * inv_r[k];
         }
     }
     if constexpr (NC == 1) {
@@ -476,9 +499,11 @@ __global__ void __launch_bounds__(256) k_moments_v(const __grid_constant__ KPara
 
 // ------------------------------------------------------------------ K2: fused stream + force + collide + boundary
 // COLL: 0 BGK, 1 MRT, 2 none (LBM_FLAG_NO_COLLIDE: pure streaming)
-template <class L, int NC, class CT, class ST, int COLL, bool BND, int VEC, bool LIST = false>
+// ZC: some component carries a Zhang-Chen weight A_kk != 0 (Eq. 11-13); built for VEC = 1 only
+template <class L, int NC, class CT, class ST, int COLL, bool BND, int VEC, bool LIST = false, bool ZC = false>
 __global__ void __launch_bounds__(128) k_step_v(const __grid_constant__ KParams<CT> p) {
     static_assert(!LIST || (BND && VEC == 1), "list mode is one cell per thread on a masked domain");
+    static_assert(!ZC || (VEC == 1 && !LIST && COLL != 2), "the Zhang-Chen variant is one cell per thread");
     unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
     if constexpr (LIST) {
         if (vid >= (unsigned)p.nfluid) return;
@@ -510,19 +535,28 @@ __global__ void __launch_bounds__(128) k_step_v(const __grid_constant__ KParams<
     if constexpr (COLL != 2) {
         // S4: F^k = -psi^k(x) sum_k' g_kk' S^k'   (Eq. 13);  du = F / rho (Eq. 5)
         CT S[NC][3][VEC], pc[NC][VEC];
+        CT Zs[ZC ? NC : 1][3][VEC];
 #pragma unroll
-        for (int kp = 0; kp < NC; ++kp) psi_sums_vec<L, CT, VEC>(p.psi + (long long)kp * p.N, c, S[kp], pc[kp]);
+        for (int kp = 0; kp < NC; ++kp) {
+            if constexpr (ZC) psi_sums_vec<L, CT, VEC, true>(p.psi + (long long)kp * p.N, c, S[kp], pc[kp], Zs[kp], p.zc_hg[kp]);
+            else psi_sums_vec<L, CT, VEC>(p.psi + (long long)kp * p.N, c, S[kp], pc[kp]);
+        }
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
             CT rc[NC], jc[NC][3], Sc[NC][3], pcc[NC], uc[3], duc[NC][3];
+            CT Zc[NC][3];
 #pragma unroll
             for (int k = 0; k < NC; ++k) {
                 rc[k] = rho[k][v];
                 pcc[k] = pc[k][v];
 #pragma unroll
-                for (int a = 0; a < 3; ++a) { jc[k][a] = j[k][a][v]; Sc[k][a] = S[k][a][v]; }
+                for (int a = 0; a < 3; ++a) {
+                    jc[k][a] = j[k][a][v]; Sc[k][a] = S[k][a][v];
+                    if constexpr (ZC) Zc[k][a] = Zs[k][a][v];
+                }
             }
-            force_and_velocity<NC, CT>(p, rc, jc, Sc, pcc, uc, duc);
+            if constexpr (ZC) force_and_velocity<NC, CT>(p, rc, jc, Sc, pcc, uc, duc, Zc);
+            else force_and_velocity<NC, CT>(p, rc, jc, Sc, pcc, uc, duc);
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 u[a][v] = uc[a];

@@ -16,6 +16,7 @@ struct LaunchArgs {
     int coll;  // 0 BGK, 1 MRT, 2 none (pure streaming)
     int vec;   // cells per thread along x in the hot kernels: 1 or vec_width<CT, ST, NC>() (needs nx % vec == 0)
     int list;  // hot kernels iterate over the fluid-cell list (one cell per thread) instead of the whole grid
+    int zc;    // a component has a Zhang-Chen weight: K2 runs its one-cell-per-thread Zhang-Chen variant
     int bnd;   // any solid cell or non-periodic axis
     const void* params;  // KParams<CT>
     const void* a0;      // op-specific (FieldIO<CT>* for init / import / export_pop; u_out for export_macro)
@@ -112,6 +113,12 @@ cudaError_t launch(const LaunchArgs& a) {
                     };
                     with_coll([&](auto C_) {
                         constexpr int VW = vec_width<CT, ST, NC>();
+                        if constexpr (C_ != 2) {
+                            if (a.zc) {
+                                k_step_v<L, NC, CT, ST, C_, (B != 0), 1, false, true><<<grid(p.N, 128), 128, 0, a.stream>>>(p);
+                                return;
+                            }
+                        }
                         if constexpr (B != 0) {
                             if (a.list) {
                                 k_step_v<L, NC, CT, ST, C_, true, 1, true><<<grid(p.nfluid, 128), 128, 0, a.stream>>>(p);

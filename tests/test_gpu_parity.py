@@ -384,3 +384,48 @@ def test_device_resident_io_and_reinit():
     assert g.steps_done == 0
     g.step(10)
     assert torch.equal(g.get_populations_device(0), f_dev)
+
+
+# ------------------------------------------------------------------ NEXT-1: A-weighted Zhang-Chen force (Eq. 11-13)
+@pytest.mark.parametrize("lattice,n,dtype", [("D2Q9", (70, 37, 1), "f64"), ("D3Q19", (22, 12, 9), "f64"), ("D3Q19", (24, 10, 9), "f32")])
+@pytest.mark.parametrize("collision", ["BGK", "MRT"])
+def test_zhang_chen_weighted_force(lattice, n, dtype, collision):
+    wl, _ = W.config1(8, dtype)
+    wl.update(lattice=lattice, nx=n[0], ny=n[1], nz=n[2], zc_A=[-0.19], collision=collision, tau=[0.9])
+    if collision == "MRT":
+        wl["mrt_rates"] = [W.mrt_rates(lattice, 0.9)]
+    inp = small_inputs(wl, 17, 0.03, 0.3)
+    o, g, fo, fg = run_pair(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
+    assert g.hot_path == "two_pass"
+    if dtype == "f64":
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+        ro, uo, po = o.get_macroscopic()
+        rg, ug, pg = g.get_macroscopic()
+        assert np.abs(uo - ug).max() <= 1e-10          # Eq. 6 velocity carries the weighted force
+        assert np.abs(po - pg).max() <= TOL64
+        assert np.abs(o.get_psi(0) - g.get_psi(0)).max() <= 1e-12 and g.get_psi(0).min() >= 0.0
+    else:
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL32, relative=True)
+
+
+def test_zhang_chen_with_walls_and_second_component():
+    """Signed-root psi storage at boundary solids (virtual density), list/dense mapping, a second component without EOS."""
+    wl, inp = W.config2(64, 32, "f64", wall=3)
+    wl.update(psi_kind=["CS", "RHO"], eos=[dict(a=W.CS_A, b=W.CS_B, R=W.CS_R, T=W.CS_T_085), dict()],
+              G=[[-1.0, 0.05], [0.05, 0.0]], zc_A=[-0.15, 0.0],
+              wetting=[dict(phi=1.1, drho=0.0, lo=0.0, hi=0.4), dict(phi=1.0, drho=0.01, lo=0.0, hi=1.0)])
+    rng = np.random.default_rng(5)
+    inp["rho"] = [0.05 + 0.25 * rng.uniform(size=64 * 32), 0.02 + 0.05 * rng.uniform(size=64 * 32)]
+    o, g, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    ro, uo, po = o.get_macroscopic()
+    rg, ug, pg = g.get_macroscopic()
+    assert np.abs(uo - ug).max() <= 1e-10
+
+
+def test_zhang_chen_needs_an_eos():
+    from paper_2506_17713_b200 import binding
+    wl, inp = W.config2(64, 32, "f64", wall=3)          # SC93 pseudopotentials
+    wl["zc_A"] = [0.2, 0.0]
+    with pytest.raises(binding.LBMError):
+        binding.LBM(wl)
