@@ -98,6 +98,7 @@ struct olbm_config {
     double mrt_rates[2][19];   // diagonal of S, moment order of R9
     double rho_ref;            // storage shift: stored = f_i - w_i*rho_ref (R16)
     double zc_A[2];            // A_kk of Eq. 11/13: F^k = A_kk F_ZC^k + (1 - A_kk) F_SC^k; 0 = pure Shan-Chen
+    double body_accel[3];      // body force per unit mass a: F^k += rho^k a (reading R19)
 };
 }
 
@@ -526,6 +527,9 @@ struct Sim : SimBase {
                     const T A = (T)c.zc_A[k];
                     for (int a = 0; a < 3; ++a) F[k][a][id] = A * (-z[a]) + (T(1) - A) * F[k][a][id];
                 }
+                // body force driving the flow: the same acceleration on every component (R19)
+                for (int a = 0; a < d; ++a)
+                    if (c.body_accel[a] != 0.0) F[k][a][id] += rho[k][id] * (T)c.body_accel[a];
             }
         }
         // S5 (R6): common velocity u' = sum_k (j^k/tau_k) / sum_k (rho^k/tau_k); = j/rho for one component

@@ -53,6 +53,7 @@ class _Config(C.Structure):
         ("mrt_rates", (C.c_double * 19) * 2),
         ("rho_ref", C.c_double),
         ("zc_A", C.c_double * 2),
+        ("body_accel", C.c_double * 3),
     ]
 
 
@@ -149,6 +150,8 @@ def make_config(wl: dict) -> _Config:
         for kp in range(nc):
             c.G[k][kp] = float(G[k][kp])
         c.zc_A[k] = float(wl.get("zc_A", [0.0] * nc)[k])
+    for a in range(3):
+        c.body_accel[a] = float(wl.get("body_accel", (0.0, 0.0, 0.0))[a])
     return c
 
 

@@ -217,3 +217,66 @@ def test_zhang_chen_weight_brings_coexistence_to_maxwell_and_conserves():
     assert abs(r[0] / W.CS_RHO_V_085 - 1) < 1.5e-2
     assert abs(rho[0].sum() / m0 - 1) < 1e-12
     assert np.abs(s.get_force(0).sum(axis=1)).max() < 1e-12
+
+
+# ------------------------------------------------------------------ NEXT-3: body force and cocurrent flow (Eq. 23)
+def test_body_force_adds_mass_times_acceleration_per_step():
+    """Periodic box, two components, interaction on: total momentum after t steps is t * (total mass) * a exactly
+    (the interaction forces cancel pairwise, the body force is rho^k a on every cell)."""
+    g = 0.4
+    a = (1e-5, -2e-5, 3e-5)
+    wl = base_wl("D3Q19", (12, 10, 8), nc=2, G=[[0.0, g], [g, 0.0]], tau=[0.8, 1.1], body_accel=a)
+    rng = np.random.default_rng(3)
+    rho = [0.5 + 0.2 * rng.uniform(size=960), 0.3 + 0.2 * rng.uniform(size=960)]
+    s = make_oracle(wl, dict(rho=rho))
+    mass = sum(r.sum() for r in rho)
+    e, w, opp = o.lattice("D3Q19")
+    t = 50
+    s.step(t)
+    mom = sum(s.get_populations(k).sum(axis=1) @ e for k in range(2))
+    assert np.abs(mom - t * mass * np.array(a)).max() < 1e-11
+
+
+def _channel(H, nx=4):
+    m = np.zeros((H + 2, nx), dtype=np.uint8)
+    m[0, :] = m[-1, :] = 1
+    return m.reshape(-1)
+
+
+def test_body_force_poiseuille_profile():
+    """Plane channel of H fluid rows between halfway bounce-back walls, single component, no interaction: the steady
+    Eq. 6 velocity is the parabola a/(2 nu) (y + 1/2)(H - 1/2 - y) (wall planes half a cell outside the fluid rows)."""
+    H, nx, tau, acc = 24, 4, 0.9, 1e-6
+    nu = (tau - 0.5) / 3.0
+    wl = base_wl("D2Q9", (nx, H + 2, 1), tau=[tau], body_accel=(acc, 0.0, 0.0))
+    s = make_oracle(wl, dict(rho=[np.ones(nx * (H + 2))], mask=_channel(H, nx)))
+    s.step(int(6 * H * H / nu))
+    u = s.get_macroscopic()[1][0].reshape(H + 2, nx)[1:-1, 0]
+    y = np.arange(H)
+    exact = acc / (2 * nu) * (y + 0.5) * (H - 0.5 - y)
+    assert np.abs(u - exact).max() < 0.01 * exact.max()
+
+
+def test_cocurrent_flow_relative_permeability_matches_eq23():
+    """layered cocurrent flow of two components (psi = rho, g_intra = -0.027, g_inter = 0.57 as in
+    P:275, both tau = 1 so M = 1), non-wetting in the centre, driven by a body force.  K_r of each phase = its flow
+    rate over the flow rate of the whole channel run single-phase (Eq. 22); Eq. 23 with M = 1."""
+    H, nx, acc = 64, 4, 2e-7
+    gi, gx = -0.027, 0.57
+    for half_width in (12, 20):
+        wl = base_wl("D2Q9", (nx, H + 2, 1), nc=2, G=[[gi, gx], [gx, gi]], tau=[1.0, 1.0], body_accel=(acc, 0.0, 0.0))
+        yy = np.repeat(np.arange(H + 2), nx)
+        centre = np.abs(yy - (H + 1) / 2) < half_width
+        rho_nw = np.where(centre, 1.0, 0.03)
+        rho_w = np.where(centre, 0.03, 1.0)
+        s = make_oracle(wl, dict(rho=[rho_nw, rho_w], mask=_channel(H, nx)))
+        s.step(40000)
+        rho, u, p = s.get_macroscopic()
+        ux = u[0].reshape(H + 2, nx)[1:-1, 0]
+        frac_nw = (rho[0] / (rho[0] + rho[1] + 1e-300)).reshape(H + 2, nx)[1:-1, 0]
+        q_total_single = acc / (2 * (1.0 / 6.0)) * H ** 3 / 6.0      # integral of the single-phase parabola over the channel
+        k_nw = (ux * frac_nw).sum() / q_total_single
+        k_w = (ux * (1 - frac_nw)).sum() / q_total_single
+        sw = 1.0 - frac_nw.sum() / H
+        assert abs(k_w - 0.5 * sw ** 2 * (3 - sw)) < 0.02
+        assert abs(k_nw - (1 - sw) * (1.5 + (1 - sw) ** 2 * (1 - 1.5))) < 0.02
