@@ -126,6 +126,7 @@ typedef struct {
     double zc_A[2];          /* A_kk of Eq. 11 / 13: F^k = A_kk F_ZC^k + (1 - A_kk) F_SC^k with the Zhang-Chen
                                 force F_ZC^k = -sum_i G_i U^k(x+e_i) e_i, U^k = alpha p_EOS - c_s^2 rho (Eq. 12).  0 = plain
                                 Shan-Chen.  Non-zero needs an EOS psi kind (LBM_E_INVALID otherwise) and runs the two-pass path. */
+    double body_accel[3];    /* body force per unit mass a: F^k += rho^k a on every fluid cell (R19) */
 } lbm_config_t;
 
 /* Bytes of device workspace lbm_create needs for cfg; 0 if cfg is invalid. */

@@ -230,6 +230,7 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
         p.wet_lo[k] = (CT)c.wet[k].lo;
         p.wet_hi[k] = (CT)c.wet[k].hi;
     }
+    for (int a = 0; a < 3; ++a) p.body[a] = (CT)(a < h->d ? c.body_accel[a] : 0.0);
     for (int fc = 0; fc < 6; ++fc) {
         p.face_kind[fc] = h->face_kind[fc];
         for (int k = 0; k < 2; ++k) p.face_rho[fc][k] = (CT)h->face_rho[fc][k];

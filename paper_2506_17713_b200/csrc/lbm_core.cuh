@@ -153,6 +153,7 @@ struct KParams {
     // U = alpha p - cs2 rho = (g_kk / 2) s |s| are available to the force without a second field.
     int zc[2];
     CT zcA[2], zc_hg[2];   // A_kk and g_kk / 2
+    CT body[3];            // body force per unit mass (R19): F^k += rho^k a, i.e. du^k += a
     int face_kind[6];
     CT face_rho[6][2];
     CT face_u[6][3];
@@ -504,6 +505,7 @@ __global__ void __launch_bounds__(128) k_export_macro(const __grid_constant__ KP
                 for (int kp = 0; kp < NC; ++kp) acc += p.G[k][kp] * S[kp][a];
                 js += j[k][a];
                 Fs += p.zc[k] ? (CT(1) - p.zcA[k]) * (-psi[k] * acc) - p.zcA[k] * Z[k][a] : -psi[k] * acc;
+                Fs += rho[k] * p.body[a];
             }
             u_out[(long long)a * p.N + id] = (js + Fs * CT(0.5)) / rt;
         }

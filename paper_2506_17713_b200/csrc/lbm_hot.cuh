@@ -444,7 +444,7 @@ __device__ __forceinline__ void force_and_velocity(const KParams<CT>& p, const C
             for (int kp = 0; kp < NC; ++kp) acc += p.G[k][kp] * S[kp][a];
             CT F = -pc[k] * acc;
             if (Z != nullptr && p.zc[k]) F = (CT(1) - p.zcA[k]) * F - p.zcA[k] * Z[k][a];
-            du[k][a] = F * inv_r[k];
+            du[k][a] = F * inv_r[k] + p.body[a];   // body force rho^k a (R19)
         }
     }
     if constexpr (NC == 1) {

@@ -429,3 +429,26 @@ def test_zhang_chen_needs_an_eos():
     wl["zc_A"] = [0.2, 0.0]
     with pytest.raises(binding.LBMError):
         binding.LBM(wl)
+
+
+# ------------------------------------------------------------------ NEXT-3: body force
+@pytest.mark.parametrize("dtype,path", [("f64", "one_pass"), ("f32", "one_pass"), ("f64", "two_pass")])
+def test_body_force_periodic_d3q19(dtype, path):
+    wl, _ = W.config5(16, dtype)
+    wl.update(nx=24, ny=10, nz=9, body_accel=(1e-4, -2e-4, 3e-4), path=path)
+    inp = small_inputs(wl, 19, 0.05, 0.3)
+    o, g, fo, fg = run_pair(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
+    assert g.hot_path == ("one_pass_ws" if path == "one_pass" else "two_pass")
+    if dtype == "f64":
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+        assert np.abs(o.get_macroscopic()[1] - g.get_macroscopic()[1]).max() <= 1e-10
+    else:
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL32, relative=True)
+
+
+def test_body_force_two_components_in_a_channel():
+    wl, inp = W.config2(64, 32, "f64", wall=3)
+    wl.update(body_accel=(2e-5, 0.0, 0.0), tau=[0.8, 1.2])
+    o, g, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    assert np.abs(o.get_macroscopic()[1] - g.get_macroscopic()[1]).max() <= 1e-10
