@@ -378,7 +378,8 @@ def main():
         if args.all_configs is None or args.all_configs:
             others = {}
             for name, k in (("C1-64", 2000), ("C2-512", 2000), ("C3-256", 100), ("C4-400-f16", 50), ("C4-400-f32", 50),
-                            ("C5-128", 500), ("C5-256", 200), ("C5-384", 100), ("C5-256-f64", 100)):
+                            ("C5-128", 500), ("C5-256", 200), ("C5-384", 100), ("C5-256-f64", 100),
+                            ("P4-416", 100)):   # the paper's own benchmark case, SURVEY 8(f) rank 4
                 try:
                     print(f"[bench] {name} ...", file=sys.stderr, flush=True)
                     rr = gpu_run(torch, name, k, 10, None, want_roofline=True, want_e2e=False)

@@ -254,6 +254,17 @@ __device__ __forceinline__ void pull(const KParams<CT>& p, const Cell& c, uint32
 }
 
 // ------------------------------------------------------------------ pseudopotential (S3)
+// Division and root of the EOS evaluation.  fp32: the hardware approximations (<= 2 ulp) -- the evaluation sits on the
+// critical path of the one-pass kernel's producers, and IEEE division / root cost ~10 instructions each; fp64: exact.
+__device__ __forceinline__ float eos_div(float a, float b) { return __fdividef(a, b); }
+__device__ __forceinline__ double eos_div(double a, double b) { return a / b; }
+__device__ __forceinline__ float eos_sqrt(float x) {
+    float r;
+    asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ double eos_sqrt(double x) { return sqrt(x); }
+
 template <class CT>
 __device__ __forceinline__ CT psi_of_rho(const KParams<CT>& p, int k, CT r) {
     const int kind = p.psi_kind[k];
@@ -265,20 +276,20 @@ __device__ __forceinline__ CT psi_of_rho(const KParams<CT>& p, int k, CT r) {
     if (kind == PSI_CS) {
         const CT eta = b * r * CT(0.25);
         const CT om = CT(1) - eta;
-        pe = r * RT * (CT(1) + eta + eta * eta - eta * eta * eta) / (om * om * om) - a * r * r;
+        pe = eos_div(r * RT * (CT(1) + eta + eta * eta - eta * eta * eta), om * om * om) - a * r * r;
     } else if (kind == PSI_PR) {
-        pe = r * RT / (CT(1) - b * r) - p.eos_aalpha[k] * r * r / (CT(1) + CT(2) * b * r - b * b * r * r);
+        pe = eos_div(r * RT, CT(1) - b * r) - eos_div(p.eos_aalpha[k] * r * r, CT(1) + CT(2) * b * r - b * b * r * r);
     } else if (kind == PSI_VDW) {
-        pe = r * RT / (CT(1) - b * r) - a * r * r;
+        pe = eos_div(r * RT, CT(1) - b * r) - a * r * r;
     } else if (kind == PSI_RK) {
-        pe = r * RT / (CT(1) - b * r) - a * r * r / (p.eos_sqrtT[k] * (CT(1) + b * r));
+        pe = eos_div(r * RT, CT(1) - b * r) - eos_div(a * r * r, p.eos_sqrtT[k] * (CT(1) + b * r));
     } else {  // PSI_RKS
-        pe = r * RT / (CT(1) - b * r) - p.eos_aalpha[k] * r * r / (CT(1) + b * r);
+        pe = eos_div(r * RT, CT(1) - b * r) - eos_div(p.eos_aalpha[k] * r * r, CT(1) + b * r);
     }
     // Eq. 12: psi = sqrt(2 (alpha p - cs2 rho) / g_kk), radicand clamped at 0 (R4); eos_inv_gkk2 = 2 / g_kk
     const CT rad = (p.eos_alpha[k] * pe - r * CT(1.0 / 3.0)) * p.eos_inv_gkk2[k];
-    if (p.zc[k]) return rad > CT(0) ? sqrt(rad) : -sqrt(-rad);   // signed root (see KParams::zc)
-    return rad > CT(0) ? sqrt(rad) : CT(0);
+    const CT sq = eos_sqrt(fabs(rad));   // one root; negative radicand: 0 (R4), or the signed root for a Zhang-Chen component
+    return rad > CT(0) ? sq : (p.zc[k] ? -sq : CT(0));
 }
 
 // f_eq (R1): w_i rho [1 + 3 e.u + 4.5 (e.u)^2 - 1.5 u.u]

@@ -353,10 +353,55 @@ constexpr int dir_of(int dx, int dy, int dz) {
 // S4 sums for VEC cells: S[a][v] = sum_i (w_i/cs2) psi(x_v + e_i) e_ia  and psi at the cells themselves.
 // rowfn(IC<dy>, IC<dz>, IC<need_x>, t, left, right) delivers psi of the row (y+dy, z+dz): t[v] at the thread's VEC
 // cells and, when need_x, the values left of lane 0 / right of lane VEC-1 (global memory in K2, shared memory in K2F).
+// S4 sums for VEC cells: S[a][v] = sum_i (w_i/cs2) psi(x_v + e_i) e_ia  and psi at the cells themselves.
+// rowfn(IC<dy>, IC<dz>, IC<need_x>, t, left, right) delivers psi of the row (y+dy, z+dz): t[v] at the thread's VEC
+// cells and, when need_x, the values left of lane 0 / right of lane VEC-1 (global memory in K2, shared memory in K2F).
+template <class L, class CT, int VEC, class RowFn>
+__device__ __forceinline__ void psi_sums_rows(RowFn&& rowfn, CT (&S)[3][VEC], CT (&pc)[VEC]) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) S[a][v] = CT(0);
+    static_for<0, 9>([&](auto RW) {
+        constexpr int dy = RW % 3 - 1, dz = RW / 3 - 1;
+        constexpr bool centre = dy == 0 && dz == 0;
+        constexpr bool has0 = row_has<L>(dy, dz, 0), hasx = row_has<L>(dy, dz, 1);
+        if constexpr ((has0 || hasx || centre) && (L::D == 3 || dz == 0)) {
+            CT t[VEC], left = CT(0), right = CT(0);
+            rowfn(IC<dy>{}, IC<dz>{}, IC<(hasx ? 1 : 0)>{}, t, left, right);
+            if constexpr (centre) {
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) pc[v] = t[v];
+            }
+            if constexpr (has0) {
+                constexpr int i = dir_of<L>(0, dy, dz);
+                constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) {
+                    if constexpr (dy != 0) S[1][v] += CT(gw * dy) * t[v];
+                    if constexpr (dz != 0) S[2][v] += CT(gw * dz) * t[v];
+                }
+            }
+            if constexpr (hasx) {
+                constexpr int i = dir_of<L>(1, dy, dz);
+                constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) {
+                    const CT m = v > 0 ? t[v - 1] : left;
+                    const CT q = v < VEC - 1 ? t[v + 1] : right;
+                    S[0][v] += gw * (q - m);
+                    if constexpr (dy != 0) S[1][v] += CT(gw * dy) * (q + m);
+                    if constexpr (dz != 0) S[2][v] += CT(gw * dz) * (q + m);
+                }
+            }
+        }
+    });
+}
+
 // ZC (Zhang-Chen weight, KParams::zc): the rows hold the signed root s; the sums use psi = max(s, 0) and
 // Zs[a][v] = sum_i (w_i/cs2) U(x_v + e_i) e_ia with U = hg s |s| is accumulated as well.
-template <class L, class CT, int VEC, bool ZC = false, class RowFn>
-__device__ __forceinline__ void psi_sums_rows(RowFn&& rowfn, CT (&S)[3][VEC], CT (&pc)[VEC], CT (*Zs)[VEC] = nullptr, CT hg = CT(0)) {
+template <class L, class CT, int VEC, bool ZC, class RowFn>
+__device__ __forceinline__ void psi_sums_rows_zc(RowFn&& rowfn, CT (&S)[3][VEC], CT (&pc)[VEC], CT (*Zs)[VEC], CT hg) {
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -417,13 +462,13 @@ __device__ __forceinline__ void psi_sums_rows(RowFn&& rowfn, CT (&S)[3][VEC], CT
 template <class L, class CT, int VEC, bool ZC = false>
 __device__ __forceinline__ void psi_sums_vec(const CT* __restrict__ ps, const VCell& c, CT (&S)[3][VEC], CT (&pc)[VEC],
                                              CT (*Zs)[VEC] = nullptr, CT hg = CT(0)) {
-    psi_sums_rows<L, CT, VEC, ZC>(
-        [&](auto DY, auto DZ, auto NX, CT (&t)[VEC], CT& left, CT& right) {
-            const CT* row = ps + (c.zo[1 + DZ] + c.yo[1 + DY]);
-            ld_vec<CT, CT, VEC>(row + c.x0, t);
-            if constexpr (NX != 0) { left = __ldg(row + c.xm); right = __ldg(row + c.xp); }
-        },
-        S, pc, Zs, hg);
+    auto rowfn = [&](auto DY, auto DZ, auto NX, CT (&t)[VEC], CT& left, CT& right) {
+        const CT* row = ps + (c.zo[1 + DZ] + c.yo[1 + DY]);
+        ld_vec<CT, CT, VEC>(row + c.x0, t);
+        if constexpr (NX != 0) { left = __ldg(row + c.xm); right = __ldg(row + c.xp); }
+    };
+    if constexpr (ZC) psi_sums_rows_zc<L, CT, VEC, true>(rowfn, S, pc, Zs, hg);
+    else psi_sums_rows<L, CT, VEC>(rowfn, S, pc);
 }
 
 // S4 + S5 for one cell: du^k = F^k / rho^k with F^k = -psi^k sum_k' g_kk' S^k' (Eq. 13, Eq. 5) and the common
