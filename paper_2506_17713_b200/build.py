@@ -30,6 +30,11 @@ def _newest_header() -> float:
 
 def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
+    # a change of compiler flags (development switches) rebuilds everything
+    stamp = OBJ / "flags.txt"
+    if not stamp.exists() or stamp.read_text() != " ".join(FLAGS):
+        force = True
+        stamp.write_text(" ".join(FLAGS))
     srcs = sorted(CSRC.glob("*.cu"))
     hdr = _newest_header()
     jobs = []

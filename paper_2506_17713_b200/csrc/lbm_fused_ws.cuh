@@ -124,7 +124,10 @@ struct WsTile {
     static constexpr size_t SMEM = sizeof(ST) * (NSTG * STAGE_ELEMS + 2 * NSTG * ROW_ELEMS) + sizeof(CT) * PSI_ELEMS + 8 * (2 * NSTG + NS + NSTG * ROWS);
     // register split: the pool is THREADS x (registers at launch)
     static constexpr int REG_LAUNCH = (65536 / THREADS) / 8 * 8;
-    static constexpr int REG_PROD = 56;
+#ifndef LBM_WS_REG_PROD
+#define LBM_WS_REG_PROD 56
+#endif
+    static constexpr int REG_PROD = LBM_WS_REG_PROD;
     static constexpr int REG_CONS_ = ((REG_LAUNCH * THREADS - REG_PROD * NPW * 32) / (NCW * 32)) / 8 * 8;
     static constexpr int REG_CONS = REG_CONS_ > 208 ? 208 : REG_CONS_;
     static_assert(SMEM <= 227 * 1024, "tile does not fit shared memory");
