@@ -527,17 +527,27 @@ void plan_fused(lbm* h) {
     const int nm = h->d == 3 ? c.nz : c.ny;
     const int tx = h->fshape.wx * 32 * h->fshape.vec;
     const long long tiles = (long long)((c.nx + tx - 1) / tx) * (h->d == 3 ? (c.ny + h->fshape.ty - 1) / h->fshape.ty : 1);
-    // aim at ~8 waves of one CTA per SM, at least 8 planes per CTA (two extra planes are pulled per chunk)
+    // Chunks per column of tiles: every CTA pulls two extra planes and pays a few planes' worth of pipeline fill, and
+    // CTAs run in waves of one per SM, so minimise  waves * (planes per chunk + 5)  (measured on 128^3 .. 512^3: the
+    // model picks 16, 128 and 128 planes, the best of the sweeps in DESIGN.md 6)
     int nsm = 148;
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
-    long long nch = (8LL * nsm + tiles - 1) / tiles;
-    nch = std::max(1LL, std::min<long long>(nch, std::max(1, nm / 8)));
-    int mchunk = (int)((nm + nch - 1) / nch);
+    long long best_cost = -1;
+    int mchunk = nm;
+    for (int nch = 1; nch <= std::max(1, nm / 8); ++nch) {
+        const int mc = (nm + nch - 1) / nch;
+        const long long ctas = tiles * ((nm + mc - 1) / mc);
+        const long long cost = ((ctas + nsm - 1) / nsm) * (mc + 5);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; mchunk = mc; }
+    }
     if (const char* e = std::getenv("LBM_TUNE_FUSED_MCHUNK")) mchunk = std::max(1, std::min(nm, std::atoi(e)));
     h->fmchunk = mchunk;
     // small domains cannot fill the GPU with marching CTAs: keep the two-pass path unless K2F is demanded
     const long long ctas = tiles * ((nm + mchunk - 1) / mchunk);
-    h->use_fused = (c.flags & LBM_FLAG_ONE_PASS) || ctas >= 2LL * nsm;
+    // ... and rows that leave more than a fifth of the lanes of the last x tile idle (measured: 96^3, 192^3 no gain)
+    const int xt = (c.nx + tx - 1) / tx;
+    const bool lanes_ok = 5 * c.nx >= 4 * xt * tx;
+    h->use_fused = (c.flags & LBM_FLAG_ONE_PASS) || (4 * ctas >= 3LL * nsm && lanes_ok);
 }
 
 Geo make_geo(const lbm* h) {
