@@ -44,6 +44,11 @@ struct lbm {
     int fmchunk;         // planes marched per CTA
     bool use_fused;      // decided in prepare()
     int last_path;       // lbm_hot_path: what the last lbm_step ran
+    // launch-bound (small) domains: GRAPH_STEPS time steps captured once into a CUDA graph and replayed
+    cudaGraphExec_t gexec;
+    int gcur;            // buffer parity the graph was captured at
+    int64_t glaunches;   // kernels per replay
+    bool gvalid, gfailed;
     bool initialized, has_solid, bnd, dirty, force_rho;
     int nbsolid;
     int nfluid;       // fluid cells (masked domains)
@@ -561,6 +566,8 @@ Geo make_geo(const lbm* h) {
 // (re)build link flags and the boundary-solid list after a mask / face change
 int prepare(lbm* h) {
     if (!h->dirty) return LBM_OK;
+    if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+    h->gvalid = false;
     h->bnd = h->has_solid || !h->cfg.periodic[0] || !h->cfg.periodic[1] || (h->d == 3 && !h->cfg.periodic[2]);
     h->nbsolid = 0;
     h->nfluid = h->N;
@@ -709,6 +716,11 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->fmchunk = 1;
     h->use_fused = false;
     h->last_path = LBM_PATH_NONE;
+    h->gexec = nullptr;
+    h->gcur = 0;
+    h->glaunches = 0;
+    h->gvalid = false;
+    h->gfailed = false;
     h->initialized = false;
     h->has_solid = false;
     h->dirty = true;
@@ -734,6 +746,7 @@ void lbm_destroy(lbm_t* h) {
     if (!h) return;
     for (auto& pr : h->ev_pending) { cudaEventDestroy(pr.a); cudaEventDestroy(pr.b); }
     for (auto e : h->ev_pool) cudaEventDestroy(e);
+    if (h->gexec) cudaGraphExecDestroy(h->gexec);
     delete h;
 }
 
@@ -827,22 +840,59 @@ int lbm_step(lbm_t* h, int n) {
     if (rc) return rc;
     if ((h->cfg.flags & LBM_FLAG_ONE_PASS) && !h->use_fused)
         return fail(h, LBM_E_UNSUPPORTED, "LBM_FLAG_ONE_PASS: the one-pass kernel does not apply to this configuration");
-    for (int s = 0; s < n; ++s) {
+    // one time step: K2F, or K1 (+K1b) + K2
+    auto step_once = [&]() -> int {
+        int r;
         if (h->use_fused) {
-            if ((rc = hot_launch(h, OP_FUSED, LBM_K_FUSED))) return rc;
-            h->cur ^= 1;
-            h->steps++;
-            continue;
+            if ((r = hot_launch(h, OP_FUSED, LBM_K_FUSED))) return r;
+        } else {
+            if (!(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) {
+                if ((r = hot_launch(h, OP_MOMENTS, LBM_K_MOMENTS))) return r;
+                if (h->nbsolid > 0 && (r = hot_launch(h, OP_VIRTUAL, LBM_K_VIRTUAL))) return r;
+            }
+            if ((r = hot_launch(h, OP_STEP, LBM_K_STEP))) return r;
+            h->last_path = LBM_PATH_TWO_PASS;
         }
-        if (!(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) {
-            if ((rc = hot_launch(h, OP_MOMENTS, LBM_K_MOMENTS))) return rc;
-            if (h->nbsolid > 0 && (rc = hot_launch(h, OP_VIRTUAL, LBM_K_VIRTUAL))) return rc;
-        }
-        if ((rc = hot_launch(h, OP_STEP, LBM_K_STEP))) return rc;
-        h->last_path = LBM_PATH_TWO_PASS;
         h->cur ^= 1;
         h->steps++;
+        return LBM_OK;
+    };
+    // Small domains are bound by kernel launches (a D2Q9 64 x 64 step is two ~3 us kernels): GRAPH_STEPS steps are
+    // captured once into a CUDA graph and replayed.  Not while profiling (event brackets), not on a stream that cannot
+    // be captured (the legacy default stream): then, and for large domains, the kernels are launched one by one.
+    constexpr int GRAPH_STEPS = 16;   // even: the ping-pong parity is the same after a replay
+    const bool small = (long long)h->N * h->cfg.n_components <= (1LL << 22);
+    if (small && !h->profiling && !h->gfailed && n >= 2 * GRAPH_STEPS + 1 && !std::getenv("LBM_TUNE_NO_GRAPH")) {
+        if ((rc = step_once())) return rc;      // first step plainly: one-time kernel attribute set-up happens outside capture
+        --n;
+        if (!h->gvalid) {
+            const int cur0 = h->cur, path0 = h->last_path;
+            const int64_t steps0 = h->steps, launches0 = h->launches;
+            cudaGraph_t graph = nullptr;
+            bool ok = cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+            if (ok) {
+                for (int s = 0; s < GRAPH_STEPS && ok; ++s) ok = step_once() == LBM_OK;
+                ok = (cudaStreamEndCapture(h->stream, &graph) == cudaSuccess) && ok && graph != nullptr;
+            }
+            if (ok) ok = cudaGraphInstantiate(&h->gexec, graph, 0) == cudaSuccess;
+            if (graph) cudaGraphDestroy(graph);
+            h->glaunches = h->launches - launches0;
+            h->cur = cur0; h->steps = steps0; h->launches = launches0; h->last_path = path0;   // nothing ran yet
+            if (ok) { h->gvalid = true; h->gcur = cur0; }
+            else { cudaGetLastError(); h->gfailed = true; h->gexec = nullptr; }
+        }
+        if (h->gvalid) {
+            if (h->cur != h->gcur) { if ((rc = step_once())) return rc; --n; }
+            while (n >= GRAPH_STEPS) {
+                CU(cudaGraphLaunch(h->gexec, h->stream));
+                h->steps += GRAPH_STEPS;
+                h->launches += h->glaunches;
+                n -= GRAPH_STEPS;
+            }
+        }
     }
+    for (int s = 0; s < n; ++s)
+        if ((rc = step_once())) return rc;
     return LBM_OK;
 }
 
