@@ -25,6 +25,8 @@
 //   A-weighted Zhang-Chen force (Eq. 11-13): F_ZC = -grad U against
 //   a re-typed EOS, weighted sum, coexistence -> Maxwell with A ~ -0.19,
 //   mass / momentum conservation.
+//   Surface-tension control (Eq. 14-16, D2Q9 MRT): sigma(kappa) / sigma(0)
+//   = 1 - kappa within 0.04 at kappa = 0.5 with the coexistence densities kept.
 //   PARITY UNPINNED: the O(u^2) terms of the pressure-face (anti-bounce-back)
 //   formula -- reading R10 -- have no paper value or closed form to be held to;
 //   see DESIGN.md.
@@ -35,6 +37,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 #include <string>
@@ -99,6 +102,7 @@ struct olbm_config {
     double rho_ref;            // storage shift: stored = f_i - w_i*rho_ref (R16)
     double zc_A[2];            // A_kk of Eq. 11/13: F^k = A_kk F_ZC^k + (1 - A_kk) F_SC^k; 0 = pure Shan-Chen
     double body_accel[3];      // body force per unit mass a: F^k += rho^k a (reading R19)
+    double st_kappa[2];        // kappa of Eq. 16: surface tension scales with 1 - kappa; D2Q9 + MRT only
 };
 }
 
@@ -587,6 +591,35 @@ struct Sim : SimBase {
                         T s = T(0);
                         for (int r_ = 0; r_ < q; ++r_) s += Minv[i][r_] * m[r_];
                         fs[i] = fi[i] - s;
+                    }
+                    // Eq. 14-16: surface-tension control, D2Q9.  Source C in moment space (Eq. 15, moment
+                    // order rho,e,eps,jx,qx,jy,qy,pxx,pxy), Q from the pseudopotential (Eq. 16, reading R20)
+                    if (c.st_kappa[k] != 0.0 && d == 2) {
+                        int xyz[3];
+                        coords(id, xyz);
+                        const T A = (T)c.zc_A[k], ps0 = psi[k][id];
+                        T Qxx = T(0), Qyy = T(0), Qxy = T(0);
+                        for (int i = 1; i < q; ++i) {
+                            const T ps1 = psi[k][scalar_nbr(xyz, i)];
+                            const T v = gw[i] * ((T(1) - A) * ps0 * (ps1 - ps0) + T(0.5) * A * (ps1 * ps1 - ps0 * ps0));
+                            Qxx += v * (T)(e[i][0] * e[i][0]);
+                            Qyy += v * (T)(e[i][1] * e[i][1]);
+                            Qxy += v * (T)(e[i][0] * e[i][1]);
+                        }
+                        // R20: Eq. 16 as printed has no interaction strength; with the factor g_kk (= -1) the
+                        // tension falls as 1 - kappa, without it it would rise
+                        const T qn = (T)c.st_kappa[k] * (T)c.G[k][k];
+                        Qxx *= qn; Qyy *= qn; Qxy *= qn;
+                        T C[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+                        C[1] = T(1.5) * (T)c.mrt_rates[k][1] * (Qxx + Qyy);
+                        C[2] = -T(1.5) * (T)c.mrt_rates[k][2] * (Qxx + Qyy);
+                        C[7] = -(T)c.mrt_rates[k][7] * (Qxx - Qyy);
+                        C[8] = -(T)c.mrt_rates[k][8] * Qxy;
+                        for (int i = 0; i < q; ++i) {
+                            T s = T(0);
+                            for (int r_ = 0; r_ < q; ++r_) s += Minv[i][r_] * C[r_];
+                            fs[i] += s;
+                        }
                     }
                 }
                 if (c.forcing == FORCE_EDM) {

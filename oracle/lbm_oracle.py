@@ -54,6 +54,7 @@ class _Config(C.Structure):
         ("rho_ref", C.c_double),
         ("zc_A", C.c_double * 2),
         ("body_accel", C.c_double * 3),
+        ("st_kappa", C.c_double * 2),
     ]
 
 
@@ -152,6 +153,8 @@ def make_config(wl: dict) -> _Config:
         c.zc_A[k] = float(wl.get("zc_A", [0.0] * nc)[k])
     for a in range(3):
         c.body_accel[a] = float(wl.get("body_accel", (0.0, 0.0, 0.0))[a])
+    for k in range(nc):
+        c.st_kappa[k] = float(wl.get("st_kappa", [0.0] * nc)[k])
     return c
 
 
