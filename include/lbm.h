@@ -127,6 +127,9 @@ typedef struct {
                                 force F_ZC^k = -sum_i G_i U^k(x+e_i) e_i, U^k = alpha p_EOS - c_s^2 rho (Eq. 12).  0 = plain
                                 Shan-Chen.  Non-zero needs an EOS psi kind (LBM_E_INVALID otherwise) and runs the two-pass path. */
     double body_accel[3];    /* body force per unit mass a: F^k += rho^k a on every fluid cell (R19) */
+    double st_kappa[2];      /* kappa of Eq. 16: MRT source term that scales the surface tension with
+                                1 - kappa and keeps the coexistence densities.  D2Q9 with LBM_MRT only (the D3Q19 form is not
+                                in the paper): LBM_E_UNSUPPORTED otherwise.  Runs the two-pass path. */
 } lbm_config_t;
 
 /* Bytes of device workspace lbm_create needs for cfg; 0 if cfg is invalid. */

@@ -49,7 +49,7 @@ class lbm_config_t(C.Structure):
         ("collision", C.c_int32), ("forcing", C.c_int32), ("compute_dtype", C.c_int32), ("store_dtype", C.c_int32),
         ("flags", C.c_uint32), ("pad_", C.c_int32),
         ("eos", lbm_eos_t * 2), ("G", (C.c_double * 2) * 2), ("wet", lbm_wetting_t * 2),
-        ("tau", C.c_double * 2), ("mrt_rates", (C.c_double * 19) * 2), ("rho_ref", C.c_double), ("zc_A", C.c_double * 2), ("body_accel", C.c_double * 3),
+        ("tau", C.c_double * 2), ("mrt_rates", (C.c_double * 19) * 2), ("rho_ref", C.c_double), ("zc_A", C.c_double * 2), ("body_accel", C.c_double * 3), ("st_kappa", C.c_double * 2),
     ]
 
 
@@ -152,6 +152,8 @@ def make_config(wl: dict) -> lbm_config_t:
         c.zc_A[k] = float(wl.get("zc_A", [0.0] * nc)[k])
     for a in range(3):
         c.body_accel[a] = float(wl.get("body_accel", (0.0, 0.0, 0.0))[a])
+    for k in range(nc):
+        c.st_kappa[k] = float(wl.get("st_kappa", [0.0] * nc)[k])
     return c
 
 

@@ -96,6 +96,7 @@ int check_config(const lbm_config_t* c) {
         }
         if (e.psi_kind == LBM_PSI_SC93 && !(e.rho0 > 0.0)) return LBM_E_INVALID;
         if (c->zc_A[k] != 0.0 && e.psi_kind > LBM_PSI_EOS_RKS) return LBM_E_INVALID;   // U of Eq. 12 needs an EOS
+        if (c->st_kappa[k] != 0.0 && (c->lattice != LBM_D2Q9 || c->collision != LBM_MRT)) return LBM_E_UNSUPPORTED;
         if (!(c->tau[k] > 0.5)) return LBM_E_INVALID;
     }
     return LBM_OK;
@@ -230,6 +231,14 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
         p.zc[k] = c.zc_A[k] != 0.0 ? 1 : 0;
         p.zcA[k] = (CT)c.zc_A[k];
         p.zc_hg[k] = (CT)(0.5 * c.G[k][k]);
+        p.st_on[k] = c.st_kappa[k] != 0.0 ? 1 : 0;
+        {
+            const double kg = c.st_kappa[k] * c.G[k][k];
+            p.st_coef[k][0] = (CT)(1.5 * c.mrt_rates[k][1] * kg);
+            p.st_coef[k][1] = (CT)(-1.5 * c.mrt_rates[k][2] * kg);
+            p.st_coef[k][2] = (CT)(-c.mrt_rates[k][7] * kg);
+            p.st_coef[k][3] = (CT)(-c.mrt_rates[k][8] * kg);
+        }
         p.wet_phi[k] = (CT)c.wet[k].phi;
         p.wet_drho[k] = (CT)c.wet[k].drho;
         p.wet_lo[k] = (CT)c.wet[k].lo;
@@ -452,7 +461,8 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.coll = (h->cfg.flags & LBM_FLAG_NO_COLLIDE) ? 2 : (h->cfg.collision == LBM_MRT ? 1 : 0);
     a.bnd = h->bnd ? 1 : 0;
     a.vec = h->vec;
-    const bool zc = h->cfg.zc_A[0] != 0.0 || (h->cfg.n_components > 1 && h->cfg.zc_A[1] != 0.0);
+    const bool zc = h->cfg.zc_A[0] != 0.0 || h->cfg.st_kappa[0] != 0.0 ||
+                    (h->cfg.n_components > 1 && (h->cfg.zc_A[1] != 0.0 || h->cfg.st_kappa[1] != 0.0));   // extended-force variant of K2
     a.zc = (zc && op == OP_STEP && !(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) ? 1 : 0;
     a.list = (h->use_list && (op == OP_MOMENTS || (op == OP_STEP && !a.zc))) ? 1 : 0;
     a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
@@ -525,7 +535,8 @@ void plan_fused(lbm* h) {
     h->use_fused = false;
     const lbm_config_t& c = h->cfg;
     if (c.flags & (LBM_FLAG_TWO_PASS | LBM_FLAG_NO_COLLIDE)) return;
-    if (c.zc_A[0] != 0.0 || (c.n_components > 1 && c.zc_A[1] != 0.0)) return;   // Zhang-Chen weight: two-pass path
+    if (c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0)))
+        return;   // Zhang-Chen weight / surface-tension source: two-pass path
     if (h->bnd || h->fshape.vec == 0 || c.nx % h->fshape.vec != 0) return;
     if ((unsigned long long)c.n_components * h->q * (unsigned long long)h->plane >= (1ULL << 32)) return;   // 32-bit element offsets
     if (h->d == 3 && c.nx % (16 / (int)h->sbytes) != 0 && h->fvariant == 0) h->fvariant = -1;   // k_fused_ws copies 16-byte pads

@@ -154,6 +154,8 @@ struct KParams {
     int zc[2];
     CT zcA[2], zc_hg[2];   // A_kk and g_kk / 2
     CT body[3];            // body force per unit mass (R19): F^k += rho^k a, i.e. du^k += a
+    int st_on[2];          // surface-tension control (Eq. 14-16): kappa != 0 (D2Q9 MRT)
+    CT st_coef[2][4];      // kappa g_kk {1.5 s_e, -1.5 s_eps, -s_nu, -s_nu} (Eq. 15 with R20)
     int face_kind[6];
     CT face_rho[6][2];
     CT face_u[6][3];

@@ -628,6 +628,35 @@ __global__ void __launch_bounds__(128) k_step_v(const __grid_constant__ KParams<
             if constexpr (COLL != 2) {
                 const CT dc[3] = {du[k][0][v], du[k][1][v], du[k][2][v]};
                 collide<L, COLL, CT>(p, k, rho[k][v], uc, dc, fc);
+                // Surface-tension control (Eq. 14-16; D2Q9 MRT, reading R20): source C in moment space from
+                // Q = kappa g_kk [(1-A) psi sum_i G_i (psi(x+e_i) - psi) e_i e_i + (A/2) sum_i G_i (psi(x+e_i)^2 - psi^2) e_i e_i]
+                if constexpr (ZC && L::D == 2 && COLL == 1) {
+                    if (p.st_on[k]) {
+                        const CT* ps = p.psi + (long long)k * p.N;
+                        auto pos = [&](CT s_) { return (p.zc[k] && s_ < CT(0)) ? CT(0) : s_; };
+                        const CT ps0 = pos(__ldg(ps + c.yo[1] + c.x0));
+                        const CT A = p.zcA[k];
+                        CT Qxx = CT(0), Qyy = CT(0), Qxy = CT(0);
+                        static_for<1, L::Q>([&](auto I) {
+                            constexpr int i = I;
+                            constexpr int ex = L::E[i][0], ey = L::E[i][1];
+                            constexpr CT gw = CT(3 * L::WN[i]) / CT(L::WD);
+                            const CT ps1 = pos(__ldg(ps + c.yo[1 + ey] + (ex == 0 ? c.x0 : (ex > 0 ? c.xp : c.xm))));
+                            const CT t = gw * ((CT(1) - A) * ps0 * (ps1 - ps0) + CT(0.5) * A * (ps1 * ps1 - ps0 * ps0));
+                            if constexpr (ex != 0) Qxx += t;
+                            if constexpr (ey != 0) Qyy += t;
+                            if constexpr (ex * ey != 0) Qxy += CT(ex * ey) * t;
+                        });
+                        // C_r (Eq. 15) for the moments e, eps, pxx, pxy; st_coef = kappa g_kk {1.5 s_e, -1.5 s_eps, -s_nu, -s_nu}
+                        const CT C1 = p.st_coef[k][0] * (Qxx + Qyy), C2 = p.st_coef[k][1] * (Qxx + Qyy);
+                        const CT C7 = p.st_coef[k][2] * (Qxx - Qyy), C8 = p.st_coef[k][3] * Qxy;
+                        static_for<0, L::Q>([&](auto I) {   // f* += M^-1 C,  M^-1 = M^T diag(1 / |row|^2) (R9)
+                            constexpr int i = I;
+                            fc[i] += C1 * (CT(mrt_entry<L>(1, i)) / CT(mrt_norm2<L>(1))) + C2 * (CT(mrt_entry<L>(2, i)) / CT(mrt_norm2<L>(2))) +
+                                     C7 * (CT(mrt_entry<L>(7, i)) / CT(mrt_norm2<L>(7))) + C8 * (CT(mrt_entry<L>(8, i)) / CT(mrt_norm2<L>(8)));
+                        });
+                    }
+                }
             }
             // links across velocity / pressure faces: the rule is applied at the writing cell (R10)
             if constexpr (BND) {

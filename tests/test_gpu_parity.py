@@ -475,3 +475,42 @@ def test_cuda_graph_replay_on_a_private_stream_matches_plain_launches():
             outs.append([s.get_populations(k) for k in range(s.nc)])
         for a, b in zip(*outs):
             assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ NEXT-2: surface-tension control (Eq. 14-16, D2Q9 MRT)
+@pytest.mark.parametrize("dtype,A", [("f64", 0.0), ("f64", -0.19), ("f32", 0.0)])
+def test_surface_tension_source_term(dtype, A):
+    wl, _ = W.config1(8, dtype)
+    wl.update(nx=70, ny=37, collision="MRT", tau=[0.9], mrt_rates=[W.mrt_rates("D2Q9", 0.9)], st_kappa=[0.5], zc_A=[A])
+    inp = small_inputs(wl, 23, 0.03, 0.3)
+    o, g, fo, fg = run_pair(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
+    assert g.hot_path == "two_pass"
+    if dtype == "f64":
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    else:
+        assert_parity(fo, fg, fluid_mask(inp, o.N), TOL32, relative=True)
+    # the source term does something: kappa = 0 gives different populations
+    o0 = make_oracle(dict(with_dtype(wl, "f64"), st_kappa=[0.0]), inp)
+    o0.step(100)
+    assert np.abs(o0.get_populations(0) - fo[0]).max() > 1e-6
+
+
+def test_surface_tension_with_walls_and_refusals():
+    from paper_2506_17713_b200 import binding
+    wl, inp = W.config2(64, 32, "f64", wall=3)
+    wl.update(psi_kind=["CS", "RHO"], eos=[dict(a=W.CS_A, b=W.CS_B, R=W.CS_R, T=W.CS_T_085), dict()],
+              G=[[-1.0, 0.05], [0.05, -0.02]], collision="MRT", tau=[1.0, 0.8],
+              mrt_rates=[W.mrt_rates("D2Q9", 1.0), W.mrt_rates("D2Q9", 0.8)], st_kappa=[0.4, 0.2],
+              wetting=[dict(phi=1.1, drho=0.0, lo=0.0, hi=0.4), dict(phi=1.0, drho=0.01, lo=0.0, hi=1.0)])
+    rng = np.random.default_rng(5)
+    inp["rho"] = [0.05 + 0.25 * rng.uniform(size=64 * 32), 0.02 + 0.05 * rng.uniform(size=64 * 32)]
+    o, g, fo, fg = run_pair(wl, inp, 100)
+    assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
+    wl3, _ = W.config5(16, "f64")                      # D3Q19: the paper does not give the source term
+    wl3.update(collision="MRT", mrt_rates=[W.mrt_rates("D3Q19", 1.0)], st_kappa=[0.5])
+    with pytest.raises(binding.LBMError):
+        binding.LBM(wl3)
+    wlb, _ = W.config1(16, "f64")                      # BGK: Eq. 14 is an MRT collision
+    wlb.update(st_kappa=[0.5])
+    with pytest.raises(binding.LBMError):
+        binding.LBM(wlb)
