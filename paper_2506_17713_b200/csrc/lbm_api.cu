@@ -563,7 +563,11 @@ void plan_fused(lbm* h) {
     // ... and rows that leave more than a fifth of the lanes of the last x tile idle (measured: 96^3, 192^3 no gain)
     const int xt = (c.nx + tx - 1) / tx;
     const bool lanes_ok = 5 * c.nx >= 4 * xt * tx;
-    h->use_fused = (c.flags & LBM_FLAG_ONE_PASS) || (4 * ctas >= 3LL * nsm && lanes_ok);
+    // By default only the warp-specialised kernel counts (D3Q19): the lock-step kernel (D2Q9, and D3Q19 rows that are not
+    // whole 16-byte vectors) is slower than the two-pass path (measured: D2Q9 4096^2 29 against 57 GMLUPS) and runs on
+    // demand only.
+    const bool ws = h->d == 3 && h->fvariant != -1;
+    h->use_fused = (c.flags & LBM_FLAG_ONE_PASS) || (ws && 4 * ctas >= 3LL * nsm && lanes_ok);
 }
 
 Geo make_geo(const lbm* h) {
