@@ -512,8 +512,9 @@ __device__ __forceinline__ void force_and_velocity(const KParams<CT>& p, const C
 
 // ------------------------------------------------------------------ K1: rho + psi
 // LIST: thread t owns the fluid cell p.flist[t] (porous domains: the dense mapping leaves most lanes on solid cells)
+// (one cell per thread -- list mode, ragged rows -- is latency-bound: cap the registers for four CTAs per SM)
 template <class L, int NC, class CT, class ST, bool BND, int VEC, bool LIST = false>
-__global__ void __launch_bounds__(256) k_moments_v(const __grid_constant__ KParams<CT> p) {
+__global__ void __launch_bounds__(256, (VEC == 1 ? 4 : 1)) k_moments_v(const __grid_constant__ KParams<CT> p) {
     static_assert(!LIST || (BND && VEC == 1), "list mode is one cell per thread on a masked domain");
     unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
     if constexpr (LIST) {
@@ -546,7 +547,7 @@ __global__ void __launch_bounds__(256) k_moments_v(const __grid_constant__ KPara
 // COLL: 0 BGK, 1 MRT, 2 none (LBM_FLAG_NO_COLLIDE: pure streaming)
 // ZC: some component carries a Zhang-Chen weight A_kk != 0 (Eq. 11-13); built for VEC = 1 only
 template <class L, int NC, class CT, class ST, int COLL, bool BND, int VEC, bool LIST = false, bool ZC = false>
-__global__ void __launch_bounds__(128) k_step_v(const __grid_constant__ KParams<CT> p) {
+__global__ void __launch_bounds__(128, ((LIST && sizeof(ST) == 2) ? 6 : 1)) k_step_v(const __grid_constant__ KParams<CT> p) {
     static_assert(!LIST || (BND && VEC == 1), "list mode is one cell per thread on a masked domain");
     static_assert(!ZC || (VEC == 1 && !LIST && COLL != 2), "the Zhang-Chen variant is one cell per thread");
     unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
