@@ -181,6 +181,21 @@ LBM_API int64_t lbm_get_boundary_solids(lbm_t* h, int64_t* out, int64_t capacity
 /* psi^k field of the current state (compute dtype converted to dtype), N values. */
 LBM_API int lbm_get_psi(lbm_t* h, int comp, void* psi, int dtype, int on_device);
 
+/* Headless in-situ rendering of the density field (PAPER.md:339, 347 render device-resident
+ * arrays without a host copy; the paper gives no formula, DESIGN.md "Rendering" is the definition).  An
+ * iso-surface rho^comp = iso seen along +axis (0 = x, 1 = y, 2 = z) with orthographic rays, one per lattice
+ * column.  Pixel (u, v): the two other axes in ascending order (axis 2: u = x, v = y; axis 1: u = x, v = z;
+ * axis 0: u = y, v = z); both images are [n_v][n_u] row-major, n_u * n_v values of dtype (LBM_F32 / LBM_F64).
+ * The field is the one lbm_get_macroscopic exports (virtual density in boundary solids, 0 in other solids).
+ * Along a ray the first pair of samples (k, k+1) with (rho_k - iso)(rho_{k+1} - iso) <= 0 and rho_k != rho_{k+1}
+ * is the hit: depth = k + (iso - rho_k) / (rho_{k+1} - rho_k); no hit: depth = -1 and shade = 0.
+ * shade = 0.1 + 0.9 max(0, n.l), n = -grad(rho)/|grad(rho)| interpolated between the two samples (central
+ * differences, periodic wrap or clamped index per axis), l = (1, 1, -2)/sqrt(6) in the (u, v, axis) frame;
+ * |grad| = 0 gives 0.1.  shade / depth: host or device pointers per on_device; either may be NULL, not both.
+ * One kernel over the resident field; nothing but the images crosses to the host. */
+LBM_API int lbm_render_isosurface(lbm_t* h, int comp, double iso, int axis, void* shade, void* depth, int dtype,
+                                  int on_device);
+
 /* Lattice tables: q, e[q][3], w[q], opposite[q].  Host pointers; any may be NULL. */
 LBM_API int lbm_get_lattice(int lattice, int* q, int* e, double* w, int* opposite);
 

@@ -73,6 +73,7 @@ _SIGNATURES = {
     "lbm_get_link_flags": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int]),
     "lbm_get_boundary_solids": (C.c_int64, [C.c_void_p, C.c_void_p, C.c_int64]),
     "lbm_get_psi": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int]),
+    "lbm_render_isosurface": (C.c_int, [C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_int]),
     "lbm_get_lattice": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "lbm_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
     "lbm_get_kernel_times": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -330,6 +331,17 @@ class LBM:
         out = np.empty(self.N, dtype=dtype)
         self._check(self.L.lbm_get_psi(self.h, k, out.ctypes.data_as(C.c_void_p), code, 0), "lbm_get_psi")
         return out
+
+    def render_isosurface(self, iso: float, axis: int = 2, k: int = 0, dtype=np.float64):
+        """(shade, depth) images [n_v, n_u] of the iso-surface rho^k = iso seen along +axis (include/lbm.h)."""
+        code = DTYPES["f32"] if dtype == np.float32 else DTYPES["f64"]
+        dims = [self.cfg.nx, self.cfg.ny, self.cfg.nz]
+        nu, nv = [dims[a] for a in range(3) if a != axis][:2]    # a bad axis is the library's to reject
+        shade = np.empty((nv, nu), dtype=dtype)
+        depth = np.empty((nv, nu), dtype=dtype)
+        self._check(self.L.lbm_render_isosurface(self.h, k, float(iso), int(axis), shade.ctypes.data_as(C.c_void_p),
+                                                 depth.ctypes.data_as(C.c_void_p), code, 0), "lbm_render_isosurface")
+        return shade, depth
 
     def set_profiling(self, enable: bool):
         self._check(self.L.lbm_set_profiling(self.h, 1 if enable else 0), "lbm_set_profiling")

@@ -369,6 +369,49 @@ __global__ void k_clamp0(CT* __restrict__ x, long long n) {
     if (i < n && x[i] < CT(0)) x[i] = CT(0);
 }
 
+// Iso-surface rendering of a resident density field (include/lbm.h: lbm_render_isosurface).  One thread per ray.
+template <typename CT>
+__global__ void k_render_iso(const CT* __restrict__ rho, int nx, int ny, int nz, int axis, int perx, int pery, int perz,
+                             CT iso, CT* __restrict__ shade, CT* __restrict__ depth) {
+    const int n[3] = {nx, ny, nz};
+    const int per[3] = {perx, pery, perz};
+    const long long st[3] = {1, nx, (long long)nx * ny};
+    const int au = axis == 0 ? 1 : 0, av = axis == 2 ? 1 : 2, aa = axis;
+    const int nu = n[au], nv = n[av], na = n[aa];
+    const long long pix = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pix >= (long long)nu * nv) return;
+    const int cu = (int)(pix % nu), cv = (int)(pix / nu);
+    const long long base = cu * st[au] + cv * st[av];
+    // central difference along axis ax at the cell with frame coordinates (cu, cv, ck)
+    auto grad = [&](int ax, int ck) -> CT {
+        const int c = ax == au ? cu : (ax == av ? cv : ck);
+        const int ip = per[ax] ? (c + 1 == n[ax] ? 0 : c + 1) : min(c + 1, n[ax] - 1);
+        const int im = per[ax] ? (c == 0 ? n[ax] - 1 : c - 1) : max(c - 1, 0);
+        const long long cell = base + ck * st[aa];
+        return CT(0.5) * (rho[cell + (ip - c) * st[ax]] - rho[cell + (im - c) * st[ax]]);
+    };
+    CT sh = 0, dp = -1;
+    CT a = rho[base];
+    for (int k = 0; k + 1 < na; ++k) {
+        const CT b = rho[base + (k + 1) * st[aa]];
+        if ((a - iso) * (b - iso) <= CT(0) && a != b) {
+            const CT w = (iso - a) / (b - a);
+            const CT gu = -((CT(1) - w) * grad(au, k) + w * grad(au, k + 1));
+            const CT gv = -((CT(1) - w) * grad(av, k) + w * grad(av, k + 1));
+            const CT ga = -((CT(1) - w) * grad(aa, k) + w * grad(aa, k + 1));
+            const CT norm = sqrt(gu * gu + gv * gv + ga * ga);
+            const CT l0 = CT(0.40824829046386301637), l2 = CT(-0.81649658092772603273);   // (1, 1, -2) / sqrt(6)
+            const CT dot = norm > CT(0) ? (gu * l0 + gv * l0 + ga * l2) / norm : CT(0);
+            sh = CT(0.1) + CT(0.9) * (dot > CT(0) ? dot : CT(0));
+            dp = CT(k) + w;
+            break;
+        }
+        a = b;
+    }
+    if (shade) shade[pix] = sh;
+    if (depth) depth[pix] = dp;
+}
+
 template <class TI, class TO>
 __global__ void k_convert(const TI* __restrict__ in, TO* __restrict__ out, long long n) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -908,6 +951,56 @@ int lbm_step(lbm_t* h, int n) {
     }
     for (int s = 0; s < n; ++s)
         if ((rc = step_once())) return rc;
+    return LBM_OK;
+}
+
+int lbm_render_isosurface(lbm_t* h, int comp, double iso, int axis, void* shade, void* depth, int dtype, int on_device) {
+    if (!h || (!shade && !depth)) return LBM_E_INVALID;
+    if (comp < 0 || comp >= h->cfg.n_components) return fail(h, LBM_E_INVALID, "component");
+    if (axis < 0 || axis > 2) return fail(h, LBM_E_INVALID, "axis");
+    if (dtype != LBM_F32 && dtype != LBM_F64) return fail(h, LBM_E_INVALID, "dtype");
+    if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_render_isosurface before lbm_init_fields");
+    int rc = prepare(h);
+    if (rc) return rc;
+    h->force_rho = true;
+    rc = do_launch(h, OP_MOMENTS);
+    h->force_rho = false;
+    if (rc) return rc;
+    if (h->nbsolid > 0 && (rc = do_launch(h, OP_VIRTUAL))) return rc;
+    const lbm_config_t& c = h->cfg;
+    const int dims[3] = {c.nx, c.ny, c.nz};
+    const long long npix = (long long)h->N / dims[axis];
+    // the images go to the free population buffer (2 fields of at most N values)
+    char* scratch = h->ws + h->cv.f[h->cur ^ 1];
+    char* sh_dev = scratch;
+    char* dp_dev = scratch + (size_t)npix * h->cbytes;
+    const char* field = h->ws + h->cv.rho + (size_t)comp * h->N * h->cbytes;
+    const unsigned grid = (unsigned)((npix + 127) / 128);
+    if (c.compute_dtype == LBM_F32)
+        k_render_iso<float><<<grid, 128, 0, h->stream>>>(reinterpret_cast<const float*>(field), c.nx, c.ny, c.nz, axis,
+                                                         c.periodic[0], c.periodic[1], c.periodic[2], (float)iso,
+                                                         reinterpret_cast<float*>(sh_dev), reinterpret_cast<float*>(dp_dev));
+    else
+        k_render_iso<double><<<grid, 128, 0, h->stream>>>(reinterpret_cast<const double*>(field), c.nx, c.ny, c.nz, axis,
+                                                          c.periodic[0], c.periodic[1], c.periodic[2], iso,
+                                                          reinterpret_cast<double*>(sh_dev), reinterpret_cast<double*>(dp_dev));
+    CU(cudaGetLastError());
+    h->launches++;
+    const size_t eb = dtype_bytes(dtype);
+    const long long chunk = std::min<long long>(npix, CHUNK_CELLS);
+    auto deliver_image = [&](const char* dev, void* dst) -> int {
+        for (long long c0 = 0; c0 < npix; c0 += chunk) {
+            const long long cnt = std::min(chunk, npix - c0);
+            int r = deliver_output(h, dev + (size_t)c0 * h->cbytes, cnt, dtype, on_device, h->ws + h->cv.stage_a,
+                                   static_cast<char*>(dst) + (size_t)c0 * eb);
+            if (r) return r;
+            if (!on_device && dtype != h->cfg.compute_dtype) CU(cudaStreamSynchronize(h->stream));
+        }
+        return LBM_OK;
+    };
+    if (shade && (rc = deliver_image(sh_dev, shade))) return rc;
+    if (depth && (rc = deliver_image(dp_dev, depth))) return rc;
+    if (!on_device) CU(cudaStreamSynchronize(h->stream));
     return LBM_OK;
 }
 
