@@ -24,7 +24,7 @@ size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 size_t dtype_bytes(int dt) { return dt == LBM_F16 ? 2 : dt == LBM_F32 ? 4 : 8; }
 
 struct Carve {
-    size_t f[2], psi, rho, flags, bsolid, flist, mask, counter, stage_a, stage_b, total;
+    size_t f[2], psi, rho, flags, bsolid, flist, nbr, mask, counter, stage_a, stage_b, total;
 };
 
 }  // namespace
@@ -53,6 +53,9 @@ struct lbm {
     int nbsolid;
     int nfluid;       // fluid cells (masked domains)
     bool use_list;    // hot kernels iterate over the fluid-cell list (porous domains)
+    bool compact_on;  // lbm_step keeps the populations in fluid-list order (lbm_compact.cuh)
+    bool is_compact;  // layout of the current population buffer
+    long long nbr_stride;
     int face_kind[6];
     double face_rho[6][2], face_u[6][3];
     int64_t steps, launches;
@@ -117,6 +120,7 @@ Carve carve(const lbm_config_t& c) {
     v.flags = take(N * 4);
     v.bsolid = take(N * 4);
     v.flist = take(N * 4 + ((N + 1023) / 1024 + 1) * 4);   // fluid-cell list + per-block counts of its compaction
+    v.nbr = take((q - 1) * (N / 4 + 64) * 4);   // neighbour table of the compact mode (fluid fraction <= 1/4)
     v.mask = take(N);
     v.counter = take(256);
     const size_t chunk = std::min<size_t>(N, CHUNK_CELLS);
@@ -184,6 +188,9 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
     p.nbsolid = h->nbsolid;
     p.flist = reinterpret_cast<const int*>(h->ws + h->cv.flist);
     p.nfluid = h->nfluid;
+    p.nbr = reinterpret_cast<const uint32_t*>(h->ws + h->cv.nbr);
+    p.nbr_stride = h->nbr_stride;
+    p.compact = 0;
     p.forcing = c.forcing == LBM_SHIFT ? 1 : 0;
     p.write_rho = (h->nbsolid > 0 || h->force_rho) ? 1 : 0;
     double w[19];
@@ -507,7 +514,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     const bool zc = h->cfg.zc_A[0] != 0.0 || h->cfg.st_kappa[0] != 0.0 ||
                     (h->cfg.n_components > 1 && (h->cfg.zc_A[1] != 0.0 || h->cfg.st_kappa[1] != 0.0));   // extended-force variant of K2
     a.zc = (zc && op == OP_STEP && !(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) ? 1 : 0;
-    a.list = (h->use_list && (op == OP_MOMENTS || (op == OP_STEP && !a.zc))) ? 1 : 0;
+    a.list = (h->use_list && (op == OP_MOMENTS || (op == OP_STEP && !a.zc))) ? (h->is_compact ? 2 : 1) : 0;
     a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
     a.variant = h->fvariant;
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;
@@ -529,6 +536,8 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
         p.f_out = h->ws + h->cv.f[out_buf];
         p.nbsolid = h->nbsolid;
         p.nfluid = h->nfluid;
+        p.nbr_stride = h->nbr_stride;
+        p.compact = h->is_compact ? 1 : 0;
         p.write_rho = (h->nbsolid > 0 || h->force_rho) ? 1 : 0;
         a.params = &p;
     };
@@ -672,6 +681,53 @@ int prepare(lbm* h) {
     h->dirty = false;
     h->params_valid = false;
     plan_fused(h);
+    // Compact mode (lbm_compact.cuh): a quarter or less of the cells fluid, plain Shan-Chen force
+    const lbm_config_t& c = h->cfg;
+    const bool ext_force = c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0));
+    h->compact_on = h->use_list && !ext_force && h->nfluid <= h->N / 4 && (long long)h->nfluid + h->nbsolid <= h->N;
+    if (const char* e = std::getenv("LBM_TUNE_COMPACT")) h->compact_on = h->compact_on && std::atoi(e) != 0;
+    if (h->compact_on) {
+        h->nbr_stride = ((long long)h->nfluid + 63) / 64 * 64;
+        int* cmap = reinterpret_cast<int*>(h->ws + h->cv.rho);   // scratch: the rho field is rewritten before it is read
+        const int* flist = reinterpret_cast<const int*>(h->ws + h->cv.flist);
+        const int* bsolid = reinterpret_cast<const int*>(h->ws + h->cv.bsolid);
+        CU(cudaMemsetAsync(cmap, 0xFF, (size_t)h->N * 4, h->stream));
+        k_cmap_scatter<<<(h->nfluid + 255) / 256, 256, 0, h->stream>>>(h->nfluid, flist, 0, cmap);
+        if (h->nbsolid > 0) k_cmap_scatter<<<(h->nbsolid + 255) / 256, 256, 0, h->stream>>>(h->nbsolid, bsolid, h->nfluid, cmap);
+        CU(cudaGetLastError());
+        h->launches += 2;
+        int rc = do_launch(h, OP_BUILD_NBR, cmap, nullptr, h->ws + h->cv.nbr);
+        if (rc) return rc;
+        CU(cudaMemsetAsync(h->ws + h->cv.rho, 0, (size_t)c.n_components * h->N * h->cbytes, h->stream));
+    }
+    return LBM_OK;
+}
+
+// Bring the current population buffer into the fluid-compact (lbm_step on porous domains) or the dense layout (every
+// other entry point): a copy through the other buffer.
+int set_layout(lbm* h, bool compact) {
+    if (!h->initialized || h->is_compact == compact) return LBM_OK;
+    const char* src = h->ws + h->cv.f[h->cur];
+    char* dst = h->ws + h->cv.f[h->cur ^ 1];
+    const int* flist = reinterpret_cast<const int*>(h->ws + h->cv.flist);
+    const int np = h->cfg.n_components * h->q;
+    const unsigned grid = (unsigned)((h->nfluid + 255) / 256);
+    int rc;
+    if (!compact) {
+        h->is_compact = false;   // the fill below is a dense kernel
+        if ((rc = do_launch(h, OP_FILL_SOLID))) return rc;
+        CU(cudaMemsetAsync(h->ws + h->cv.psi, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
+    }
+    if (h->sbytes == 2)
+        k_pack<uint16_t><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint16_t*>(src), reinterpret_cast<uint16_t*>(dst), flist, h->nfluid, h->plane, np, compact ? 0 : 1);
+    else if (h->sbytes == 4)
+        k_pack<uint32_t><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint32_t*>(src), reinterpret_cast<uint32_t*>(dst), flist, h->nfluid, h->plane, np, compact ? 0 : 1);
+    else
+        k_pack<unsigned long long><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const unsigned long long*>(src), reinterpret_cast<unsigned long long*>(dst), flist, h->nfluid, h->plane, np, compact ? 0 : 1);
+    CU(cudaGetLastError());
+    h->launches++;
+    h->cur ^= 1;
+    h->is_compact = compact;
     return LBM_OK;
 }
 
@@ -786,6 +842,9 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->force_rho = false;
     h->nbsolid = 0;
     h->nfluid = h->N;
+    h->compact_on = false;
+    h->is_compact = false;
+    h->nbr_stride = 0;
     h->use_list = false;
     h->steps = 0;
     h->launches = 0;
@@ -857,6 +916,7 @@ int lbm_init_fields(lbm_t* h, const void* const* rho, const void* u, int dtype, 
     if (dtype != LBM_F32 && dtype != LBM_F64) return fail(h, LBM_E_INVALID, "dtype");
     int rc = prepare(h);
     if (rc) return rc;
+    h->is_compact = false;   // whatever the buffers held is overwritten in the dense layout
     const int nc = h->cfg.n_components;
     for (int k = 0; k < nc; ++k)
         if (!rho[k]) return fail(h, LBM_E_INVALID, "rho[k] is NULL");
@@ -896,6 +956,7 @@ int lbm_step(lbm_t* h, int n) {
     if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_step before lbm_init_fields");
     int rc = prepare(h);
     if (rc) return rc;
+    if ((rc = set_layout(h, h->compact_on))) return rc;
     if ((h->cfg.flags & LBM_FLAG_ONE_PASS) && !h->use_fused)
         return fail(h, LBM_E_UNSUPPORTED, "LBM_FLAG_ONE_PASS: the one-pass kernel does not apply to this configuration");
     // one time step: K2F, or K1 (+K1b) + K2
@@ -909,7 +970,7 @@ int lbm_step(lbm_t* h, int n) {
                 if (h->nbsolid > 0 && (r = hot_launch(h, OP_VIRTUAL, LBM_K_VIRTUAL))) return r;
             }
             if ((r = hot_launch(h, OP_STEP, LBM_K_STEP))) return r;
-            h->last_path = LBM_PATH_TWO_PASS;
+            h->last_path = h->is_compact ? LBM_PATH_TWO_PASS_COMPACT : LBM_PATH_TWO_PASS;
         }
         h->cur ^= 1;
         h->steps++;
@@ -962,6 +1023,7 @@ int lbm_render_isosurface(lbm_t* h, int comp, double iso, int axis, void* shade,
     if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_render_isosurface before lbm_init_fields");
     int rc = prepare(h);
     if (rc) return rc;
+    if ((rc = set_layout(h, false))) return rc;
     h->force_rho = true;
     rc = do_launch(h, OP_MOMENTS);
     h->force_rho = false;
@@ -1010,6 +1072,7 @@ int lbm_get_macroscopic(lbm_t* h, void* const* rho, void* u, void* p, int dtype,
     if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_get_macroscopic before lbm_init_fields");
     int rc = prepare(h);
     if (rc) return rc;
+    if ((rc = set_layout(h, false))) return rc;
     const int nc = h->cfg.n_components;
     // refresh rho / psi of the current state: K1 (with rho output) and K1b
     h->force_rho = true;
@@ -1056,6 +1119,7 @@ int lbm_get_populations(lbm_t* h, int comp, void* f, int dtype, int on_device) {
     if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_get_populations before lbm_init_fields");
     int rc = prepare(h);
     if (rc) return rc;
+    if ((rc = set_layout(h, false))) return rc;
     const size_t eb = dtype_bytes(dtype);
     if (on_device && dtype == h->cfg.compute_dtype) {  // straight into the caller's array
         FieldIOAny io;
@@ -1089,6 +1153,7 @@ int lbm_set_populations(lbm_t* h, int comp, const void* f, int dtype, int on_dev
     if (h->steps != 0) return fail(h, LBM_E_STATE, "lbm_set_populations is only valid right after lbm_init_fields");
     int rc = prepare(h);
     if (rc) return rc;
+    if ((rc = set_layout(h, false))) return rc;
     const size_t eb = dtype_bytes(dtype);
     const int chunk = std::min(h->N, CHUNK_CELLS);
     for (int c0 = 0; c0 < h->N; c0 += chunk) {
@@ -1153,6 +1218,7 @@ int lbm_get_psi(lbm_t* h, int comp, void* psi, int dtype, int on_device) {
     if (!h->initialized) return fail(h, LBM_E_STATE, "lbm_get_psi before lbm_init_fields");
     int rc = prepare(h);
     if (rc) return rc;
+    if ((rc = set_layout(h, false))) return rc;
     if ((rc = do_launch(h, OP_MOMENTS))) return rc;
     if (h->nbsolid > 0 && (rc = do_launch(h, OP_VIRTUAL))) return rc;
     if (h->cfg.zc_A[comp] != 0.0) {   // the next lbm_step recomputes the field anyway

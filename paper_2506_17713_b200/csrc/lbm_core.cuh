@@ -135,6 +135,10 @@ struct KParams {
     int nbsolid;
     const int* flist;  // fluid-cell list, ascending (list mode of the hot kernels on porous domains)
     int nfluid;
+    // compact mode (lbm_compact.cuh): neighbour table [(Q-1)][nbr_stride] of extended indices; psi in extended order
+    const uint32_t* nbr;
+    long long nbr_stride;
+    int compact;
     // mode
     int forcing;       // 0 EDM, 1 SHIFT
     int write_rho;     // K1 also writes rho (needed by K1b and the exports)
@@ -340,7 +344,7 @@ __global__ void __launch_bounds__(128) k_virtual_density(const __grid_constant__
         rs = rs < p.wet_lo[k] ? p.wet_lo[k] : rs;
         rs = rs > p.wet_hi[k] ? p.wet_hi[k] : rs;
         p.rho[(long long)k * p.N + id] = rs;
-        p.psi[(long long)k * p.N + id] = psi_of_rho(p, k, rs);
+        p.psi[(long long)k * p.N + (p.compact ? p.nfluid + b : id)] = psi_of_rho(p, k, rs);
     }
 }
 

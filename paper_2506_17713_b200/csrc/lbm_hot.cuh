@@ -510,6 +510,35 @@ __device__ __forceinline__ void force_and_velocity(const KParams<CT>& p, const C
     }
 }
 
+// Links of a fluid cell that cross a velocity / pressure face: the rule is applied at the writing cell (R10), on the
+// post-collision populations fc of component k; uc = common velocity of the cell.
+template <class L, class CT>
+__device__ __forceinline__ void apply_face_rules(const KParams<CT>& p, const Cell& cc, int k, const CT (&uc)[3], CT (&fc)[L::Q]) {
+    const CT uu15 = CT(1.5) * (uc[0] * uc[0] + uc[1] * uc[1] + uc[2] * uc[2]);
+    static_for<1, L::Q>([&](auto O) {
+        constexpr int o = O;
+        constexpr int eox = L::E[o][0], eoy = L::E[o][1], eoz = L::E[o][2];
+        constexpr CT w = CT(L::WN[o]) / CT(L::WD);
+        const int face = crossed_face<L, o>(p, cc);
+        if (face >= 0) {
+            const int kind = p.face_kind[face];
+            if (kind == FACE_VELOCITY) {   // arriving direction i = opposite(o), e_i = -e_o
+                CT eu = CT(0);
+                if constexpr (eox != 0) eu -= CT(eox) * p.face_u[face][0];
+                if constexpr (eoy != 0) eu -= CT(eoy) * p.face_u[face][1];
+                if constexpr (eoz != 0) eu -= CT(eoz) * p.face_u[face][2];
+                fc[o] = fc[o] + CT(2) * w * p.face_rho[face][k] * eu * CT(3);
+            } else if (kind == FACE_PRESSURE) {
+                CT eu = CT(0);
+                if constexpr (eox != 0) eu += CT(eox) * uc[0];
+                if constexpr (eoy != 0) eu += CT(eoy) * uc[1];
+                if constexpr (eoz != 0) eu += CT(eoz) * uc[2];
+                fc[o] = -fc[o] + CT(2) * w * p.face_rho[face][k] * (CT(1) + CT(4.5) * eu * eu - uu15);
+            }
+        }
+    });
+}
+
 // ------------------------------------------------------------------ K1: rho + psi
 // LIST: thread t owns the fluid cell p.flist[t] (porous domains: the dense mapping leaves most lanes on solid cells)
 // (one cell per thread -- list mode, ragged rows -- is latency-bound: cap the registers for four CTAs per SM)
@@ -664,29 +693,7 @@ __global__ void __launch_bounds__(128, ((LIST && sizeof(ST) == 2) ? 6 : 1)) k_st
                 if (fl[v] & FACEBC_BIT) {
                     Cell cc;
                     cc.x = c.x0 + v; cc.y = c.y; cc.z = c.z;
-                    const CT uu15 = CT(1.5) * (uc[0] * uc[0] + uc[1] * uc[1] + uc[2] * uc[2]);
-                    static_for<1, L::Q>([&](auto O) {
-                        constexpr int o = O;
-                        constexpr int eox = L::E[o][0], eoy = L::E[o][1], eoz = L::E[o][2];
-                        constexpr CT w = CT(L::WN[o]) / CT(L::WD);
-                        const int face = crossed_face<L, o>(p, cc);
-                        if (face >= 0) {
-                            const int kind = p.face_kind[face];
-                            if (kind == FACE_VELOCITY) {   // arriving direction i = opposite(o), e_i = -e_o
-                                CT eu = CT(0);
-                                if constexpr (eox != 0) eu -= CT(eox) * p.face_u[face][0];
-                                if constexpr (eoy != 0) eu -= CT(eoy) * p.face_u[face][1];
-                                if constexpr (eoz != 0) eu -= CT(eoz) * p.face_u[face][2];
-                                fc[o] = fc[o] + CT(2) * w * p.face_rho[face][k] * eu * CT(3);
-                            } else if (kind == FACE_PRESSURE) {
-                                CT eu = CT(0);
-                                if constexpr (eox != 0) eu += CT(eox) * uc[0];
-                                if constexpr (eoy != 0) eu += CT(eoy) * uc[1];
-                                if constexpr (eoz != 0) eu += CT(eoz) * uc[2];
-                                fc[o] = -fc[o] + CT(2) * w * p.face_rho[face][k] * (CT(1) + CT(4.5) * eu * eu - uu15);
-                            }
-                        }
-                    });
+                    apply_face_rules<L, CT>(p, cc, k, uc, fc);
                 }
             }
             static_for<0, L::Q>([&](auto I) { f[k][I][v] = fc[I] - p.wref[I]; });

@@ -5,17 +5,20 @@
 #include <cstdlib>
 #include "lbm_fused.cuh"
 #include "lbm_fused_ws.cuh"
+#include "lbm_compact.cuh"
 
 namespace lbmk {
 
-enum Op { OP_MOMENTS = 0, OP_VIRTUAL = 1, OP_STEP = 2, OP_INIT = 3, OP_EXPORT_MACRO = 4, OP_EXPORT_POP = 5, OP_IMPORT_POP = 6, OP_UNSTREAM = 7, OP_FUSED = 8 };
+enum Op { OP_MOMENTS = 0, OP_VIRTUAL = 1, OP_STEP = 2, OP_INIT = 3, OP_EXPORT_MACRO = 4, OP_EXPORT_POP = 5, OP_IMPORT_POP = 6, OP_UNSTREAM = 7, OP_FUSED = 8,
+          OP_BUILD_NBR = 9 /* a0 = dense -> extended index map, a2 = table */, OP_FILL_SOLID = 10 };
 
 struct LaunchArgs {
     int op;
     int nc;    // components
     int coll;  // 0 BGK, 1 MRT, 2 none (pure streaming)
     int vec;   // cells per thread along x in the hot kernels: 1 or vec_width<CT, ST, NC>() (needs nx % vec == 0)
-    int list;  // hot kernels iterate over the fluid-cell list (one cell per thread) instead of the whole grid
+    int list;  // 1: hot kernels iterate over the fluid-cell list (one cell per thread) instead of the whole grid;
+               // 2: compact mode, populations in fluid-list order (lbm_compact.cuh)
     int zc;    // a component has a Zhang-Chen weight: K2 runs its one-cell-per-thread Zhang-Chen variant
     int bnd;   // any solid cell or non-periodic axis
     const void* params;  // KParams<CT>
@@ -87,6 +90,10 @@ cudaError_t launch(const LaunchArgs& a) {
                 with_bnd([&](auto B) {
                     constexpr int VW = vec_width<CT, ST, NC>();
                     if constexpr (B != 0) {
+                        if (a.list == 2) {
+                            k_moments_c<L, NC, CT, ST><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p);
+                            return;
+                        }
                         if (a.list) {
                             k_moments_v<L, NC, CT, ST, true, 1, true><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p);
                             return;
@@ -120,6 +127,10 @@ cudaError_t launch(const LaunchArgs& a) {
                             }
                         }
                         if constexpr (B != 0) {
+                            if (a.list == 2) {
+                                k_step_c<L, NC, CT, ST, C_><<<grid(p.nfluid, 128), 128, 0, a.stream>>>(p);
+                                return;
+                            }
                             if (a.list) {
                                 k_step_v<L, NC, CT, ST, C_, true, 1, true><<<grid(p.nfluid, 128), 128, 0, a.stream>>>(p);
                                 return;
@@ -132,6 +143,12 @@ cudaError_t launch(const LaunchArgs& a) {
                     });
                 });
             });
+            break;
+        case OP_BUILD_NBR:
+            k_build_nbr<L, CT><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p, static_cast<const int*>(a.a0), static_cast<uint32_t*>(a.a2));
+            break;
+        case OP_FILL_SOLID:
+            with_nc([&](auto NC) { k_fill_solid<L, NC, CT, ST><<<grid(p.N, 256), 256, 0, a.stream>>>(p); });
             break;
         case OP_UNSTREAM:
             with_nc([&](auto NC) {
