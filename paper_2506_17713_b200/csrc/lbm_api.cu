@@ -324,9 +324,10 @@ __global__ void k_list_boundary_solids(Geo g, const uint32_t* __restrict__ flags
 
 // Fluid-cell list in ascending order (stream compaction in three small kernels: per-block counts, scan, fill).
 constexpr int COMPACT_BLOCK = 1024;
-__global__ void __launch_bounds__(COMPACT_BLOCK) k_fluid_count(int N, const uint32_t* __restrict__ flags, int* __restrict__ blockcnt) {
+__global__ void __launch_bounds__(COMPACT_BLOCK) k_fluid_count(int N, const uint32_t* __restrict__ flags, int* __restrict__ blockcnt,
+                                                               uint32_t tmask = SOLID_BIT, uint32_t tval = 0u) {
     const int id = blockIdx.x * COMPACT_BLOCK + threadIdx.x;
-    const int fluid = id < N && !(flags[id] & SOLID_BIT);
+    const int fluid = id < N && (flags[id] & tmask) == tval;   // default predicate: fluid cell
     const int n = __syncthreads_count(fluid);
     if (threadIdx.x == 0) blockcnt[blockIdx.x] = n;
 }
@@ -351,10 +352,10 @@ __global__ void __launch_bounds__(1024) k_fluid_scan(int nb, int* __restrict__ b
     if (t == 1023) blockcnt[nb] = part[1023];
 }
 __global__ void __launch_bounds__(COMPACT_BLOCK) k_fluid_fill(int N, const uint32_t* __restrict__ flags, const int* __restrict__ blockoff,
-                                                              int* __restrict__ list) {
+                                                              int* __restrict__ list, uint32_t tmask = SOLID_BIT, uint32_t tval = 0u) {
     __shared__ int wcnt[COMPACT_BLOCK / 32];
     const int id = blockIdx.x * COMPACT_BLOCK + threadIdx.x;
-    const int fluid = id < N && !(flags[id] & SOLID_BIT);
+    const int fluid = id < N && (flags[id] & tmask) == tval;
     const unsigned bal = __ballot_sync(0xffffffffu, fluid);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     if (lane == 0) wcnt[w] = __popc(bal);
@@ -362,6 +363,11 @@ __global__ void __launch_bounds__(COMPACT_BLOCK) k_fluid_fill(int N, const uint3
     int off = blockoff[blockIdx.x];
     for (int k = 0; k < w; ++k) off += wcnt[k];
     if (fluid) list[off + __popc(bal & ((1u << lane) - 1u))] = id;
+}
+
+__global__ void k_mark(int n, const int* __restrict__ list, uint32_t* __restrict__ marks) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n) marks[list[t]] = 1u;
 }
 
 __global__ void k_export_flags(int N, const uint32_t* __restrict__ in, uint32_t* __restrict__ out) {
@@ -673,6 +679,20 @@ int prepare(lbm* h) {
             CU(cudaStreamSynchronize(h->stream));
             h->nbsolid = cnt[0];
             h->nfluid = cnt[1];
+            if (h->nbsolid > 0) {
+                // the atomic append left the boundary solids in arbitrary order: rewrite the list in ascending cell order
+                // (deterministic; neighbouring threads of K1b, and the psi gathers of the compact mode, then touch
+                // neighbouring memory).  Scratch: the rho field (zeroed again below).
+                uint32_t* marks = reinterpret_cast<uint32_t*>(h->ws + h->cv.rho);
+                CU(cudaMemsetAsync(marks, 0, (size_t)h->N * 4, h->stream));
+                k_mark<<<(h->nbsolid + 255) / 256, 256, 0, h->stream>>>(h->nbsolid, list, marks);
+                k_fluid_count<<<nb, COMPACT_BLOCK, 0, h->stream>>>(h->N, marks, blockcnt, 1u, 1u);
+                k_fluid_scan<<<1, 1024, 0, h->stream>>>(nb, blockcnt);
+                k_fluid_fill<<<nb, COMPACT_BLOCK, 0, h->stream>>>(h->N, marks, blockcnt, list, 1u, 1u);
+                CU(cudaGetLastError());
+                h->launches += 4;
+                CU(cudaMemsetAsync(h->ws + h->cv.rho, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
+            }
             // with most cells solid the dense mapping wastes lanes and issue slots on them: one thread per fluid cell
             h->use_list = h->nfluid < h->N / 2;
             if (const char* e = std::getenv("LBM_TUNE_LIST")) h->use_list = std::atoi(e) != 0;

@@ -121,18 +121,34 @@ __global__ void __launch_bounds__(256, 4) k_moments_c(const __grid_constant__ KP
 }
 
 // ------------------------------------------------------------------ K2 in compact order
+// One cell per thread and gathers everywhere: the kernel lives on warps in flight.  With two components the 2 x Q
+// pulled populations are parked in shared memory ([component][direction][thread], conflict-free, private to the
+// thread: no barrier) between the moment sums and the collision, which keeps the kernel at 64 .. 100 registers
+// (five to eight CTAs per SM instead of four at 128 registers).
+#ifndef LBM_COMPACT_PARK
+#define LBM_COMPACT_PARK 1
+#endif
+// CTAs per SM (measured on config 4, 400^3: fp32 store 1.46 ms at 5 against 1.52 at 8; fp16 store 1.29 at 8, 1.41 at 5)
+#ifndef LBM_COMPACT_CTAS
+#define LBM_COMPACT_CTAS (sizeof(ST) == 2 ? 8 : 5)
+#endif
 template <class L, int NC, class CT, class ST, int COLL>
-__global__ void __launch_bounds__(128, (sizeof(ST) == 2 ? 6 : 1)) k_step_c(const __grid_constant__ KParams<CT> p) {
+__global__ void __launch_bounds__(128, ((NC == 2 && LBM_COMPACT_PARK) || sizeof(ST) == 2 ? LBM_COMPACT_CTAS : 1))
+k_step_c(const __grid_constant__ KParams<CT> p) {
+    constexpr bool PARK = NC == 2 && LBM_COMPACT_PARK;
+    __shared__ CT park[PARK ? NC * L::Q * 128 : 1];
     const unsigned n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= (unsigned)p.nfluid) return;
     uint32_t nb[L::Q];
     load_nbr<L, CT>(p, n, nb);
 
-    CT f[NC][L::Q], rho[NC], j[NC][3];
+    CT f[PARK ? 1 : NC][L::Q], rho[NC], j[NC][3];
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
-        pull_compact<L, CT, ST>(p, n, nb, k, f[k]);
-        if constexpr (COLL != 2) moments<L, CT>(f[k], rho[k], j[k]);
+        CT(&fk)[L::Q] = f[PARK ? 0 : k];
+        pull_compact<L, CT, ST>(p, n, nb, k, fk);
+        if constexpr (COLL != 2) moments<L, CT>(fk, rho[k], j[k]);
+        if constexpr (PARK) static_for<0, L::Q>([&](auto I) { park[(k * L::Q + I) * 128 + threadIdx.x] = fk[I]; });
     }
     CT u[3] = {CT(0), CT(0), CT(0)}, du[NC][3];
     if constexpr (COLL != 2) {
@@ -164,17 +180,19 @@ __global__ void __launch_bounds__(128, (sizeof(ST) == 2 ? 6 : 1)) k_step_c(const
     static_for<1, L::Q>([&](auto I) { anyface |= nb[I]; });
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
-        if constexpr (COLL != 2) collide<L, COLL, CT>(p, k, rho[k], u, du[k], f[k]);
+        CT(&fk)[L::Q] = f[PARK ? 0 : k];
+        if constexpr (PARK) static_for<0, L::Q>([&](auto I) { fk[I] = park[(k * L::Q + I) * 128 + threadIdx.x]; });
+        if constexpr (COLL != 2) collide<L, COLL, CT>(p, k, rho[k], u, du[k], fk);
         if (anyface & NBR_FACE) {   // a link of this cell crosses a non-periodic face: velocity / pressure rules (R10)
             const int id = __ldg(p.flist + n);
             if (__ldg(p.flags + id) & FACEBC_BIT) {
                 Cell cc;
                 cc.x = id % p.nx; cc.y = (id / p.nx) % p.ny; cc.z = id / (p.nx * p.ny);
-                apply_face_rules<L, CT>(p, cc, k, u, f[k]);
+                apply_face_rules<L, CT>(p, cc, k, u, fk);
             }
         }
         ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.plane + n;
-        static_for<0, L::Q>([&](auto I) { Conv<CT, ST>::st(out + (long long)I * p.plane, f[k][I] - p.wref[I]); });
+        static_for<0, L::Q>([&](auto I) { Conv<CT, ST>::st(out + (long long)I * p.plane, fk[I] - p.wref[I]); });
     }
 }
 
