@@ -190,6 +190,7 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
     p.nfluid = h->nfluid;
     p.nbr = reinterpret_cast<const uint32_t*>(h->ws + h->cv.nbr);
     p.nbr_stride = h->nbr_stride;
+    p.cplane = h->nbr_stride;
     p.compact = 0;
     p.forcing = c.forcing == LBM_SHIFT ? 1 : 0;
     p.write_rho = (h->nbsolid > 0 || h->force_rho) ? 1 : 0;
@@ -543,6 +544,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
         p.nbsolid = h->nbsolid;
         p.nfluid = h->nfluid;
         p.nbr_stride = h->nbr_stride;
+        p.cplane = h->nbr_stride;
         p.compact = h->is_compact ? 1 : 0;
         p.write_rho = (h->nbsolid > 0 || h->force_rho) ? 1 : 0;
         a.params = &p;
@@ -706,6 +708,8 @@ int prepare(lbm* h) {
     const bool ext_force = c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0));
     h->compact_on = h->use_list && !ext_force && h->nfluid <= h->N / 4 && (long long)h->nfluid + h->nbsolid <= h->N;
     if (const char* e = std::getenv("LBM_TUNE_COMPACT")) h->compact_on = h->compact_on && std::atoi(e) != 0;
+    if (h->compact_on && (unsigned long long)h->q * (((unsigned long long)h->nfluid + 63) / 64 * 64) >= (1ULL << 32))
+        h->compact_on = false;   // 32-bit element offsets within a component
     if (h->compact_on) {
         h->nbr_stride = ((long long)h->nfluid + 63) / 64 * 64;
         int* cmap = reinterpret_cast<int*>(h->ws + h->cv.rho);   // scratch: the rho field is rewritten before it is read
@@ -739,11 +743,11 @@ int set_layout(lbm* h, bool compact) {
         CU(cudaMemsetAsync(h->ws + h->cv.psi, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
     }
     if (h->sbytes == 2)
-        k_pack<uint16_t><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint16_t*>(src), reinterpret_cast<uint16_t*>(dst), flist, h->nfluid, h->plane, np, compact ? 0 : 1);
+        k_pack<uint16_t><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint16_t*>(src), reinterpret_cast<uint16_t*>(dst), flist, h->nfluid, h->plane, h->nbr_stride, np, compact ? 0 : 1);
     else if (h->sbytes == 4)
-        k_pack<uint32_t><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint32_t*>(src), reinterpret_cast<uint32_t*>(dst), flist, h->nfluid, h->plane, np, compact ? 0 : 1);
+        k_pack<uint32_t><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint32_t*>(src), reinterpret_cast<uint32_t*>(dst), flist, h->nfluid, h->plane, h->nbr_stride, np, compact ? 0 : 1);
     else
-        k_pack<unsigned long long><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const unsigned long long*>(src), reinterpret_cast<unsigned long long*>(dst), flist, h->nfluid, h->plane, np, compact ? 0 : 1);
+        k_pack<unsigned long long><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const unsigned long long*>(src), reinterpret_cast<unsigned long long*>(dst), flist, h->nfluid, h->plane, h->nbr_stride, np, compact ? 0 : 1);
     CU(cudaGetLastError());
     h->launches++;
     h->cur ^= 1;

@@ -2,7 +2,8 @@
 //
 // With most cells solid (config 4: 77 %), the dense [cell] planes spend most of every 32-byte sector on solid slots that
 // nobody reads.  While lbm_step runs on such a domain the populations therefore live in the order of the fluid-cell list:
-// slot n of a direction plane belongs to the n-th fluid cell (ascending cell index), and psi lives in "extended" order
+// slot n of a direction plane belongs to the n-th fluid cell (ascending cell index; the planes are cplane = nfluid rounded
+// up to 64 elements apart, so the whole state is one contiguous block), and psi lives in "extended" order
 // (slots [0, nfluid) = fluid cells, [nfluid, nfluid + nbsolid) = boundary solids in the order of their list).  One
 // neighbour table nbr[(i-1) * nbr_stride + n] (i = 1 .. Q-1) holds the extended index of the cell at x + e_i (wrap, or the
 // clamped cell of R10 with bit 31 set when the link crosses a non-periodic face).  It serves both stencils:
@@ -54,12 +55,13 @@ static __global__ void __launch_bounds__(256) k_cmap_scatter(int n, const int* _
 // dense -> compact / compact -> dense copies of every population plane (T = raw storage element)
 template <class T>
 __global__ void __launch_bounds__(256) k_pack(const T* __restrict__ src, T* __restrict__ dst, const int* __restrict__ flist,
-                                             int nfluid, long long plane, int nplanes, int to_dense) {
+                                             int nfluid, long long plane, long long cplane, int nplanes, int to_dense) {
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= nfluid) return;
     const int id = __ldg(flist + n);
     const long long from = to_dense ? n : id, to = to_dense ? id : n;
-    for (int pl = 0; pl < nplanes; ++pl) dst[pl * plane + to] = src[pl * plane + from];
+    const long long sp = to_dense ? cplane : plane, dp = to_dense ? plane : cplane;
+    for (int pl = 0; pl < nplanes; ++pl) dst[pl * dp + to] = src[pl * sp + from];
 }
 
 // solid cells of the dense layout hold f_eq(1, 0) (include/lbm.h, lbm_init_fields)
@@ -88,7 +90,9 @@ __device__ __forceinline__ void load_nbr(const KParams<CT>& p, unsigned n, uint3
 // S7 read side in compact order: f[i] = stored_i(x - e_i), or stored_ibar(x) on a flagged link
 template <class L, class CT, class ST>
 __device__ __forceinline__ void pull_compact(const KParams<CT>& p, unsigned n, const uint32_t (&nb)[L::Q], int k, CT (&f)[L::Q]) {
-    const ST* base = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.plane;
+    // 32-bit element offsets within a component (Q * cplane < 2^32 is a condition of the mode)
+    const ST* base = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.cplane;
+    const uint32_t cp = (uint32_t)p.cplane;
     static_for<0, L::Q>([&](auto I) {
         constexpr int i = I;
         if constexpr (i == 0) {
@@ -97,7 +101,8 @@ __device__ __forceinline__ void pull_compact(const KParams<CT>& p, unsigned n, c
             constexpr int ib = opposite<L>(i);
             const uint32_t s = nb[ib];
             const bool ok = s < (uint32_t)p.nfluid;
-            f[i] = ld_one<CT, ST>(base + (long long)(ok ? i : ib) * p.plane + (ok ? s : n)) + p.wref[i];
+            const uint32_t off = ok ? (uint32_t)i * cp + s : (uint32_t)ib * cp + n;
+            f[i] = ld_one<CT, ST>(base + off) + p.wref[i];
         }
     });
 }
@@ -191,8 +196,9 @@ k_step_c(const __grid_constant__ KParams<CT> p) {
                 apply_face_rules<L, CT>(p, cc, k, u, fk);
             }
         }
-        ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.plane + n;
-        static_for<0, L::Q>([&](auto I) { Conv<CT, ST>::st(out + (long long)I * p.plane, fk[I] - p.wref[I]); });
+        ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.cplane;
+        const uint32_t cp = (uint32_t)p.cplane;
+        static_for<0, L::Q>([&](auto I) { Conv<CT, ST>::st(out + ((uint32_t)I * cp + n), fk[I] - p.wref[I]); });
     }
 }
 

@@ -138,6 +138,7 @@ struct KParams {
     // compact mode (lbm_compact.cuh): neighbour table [(Q-1)][nbr_stride] of extended indices; psi in extended order
     const uint32_t* nbr;
     long long nbr_stride;
+    long long cplane;   // elements between consecutive direction planes in compact order (= nbr_stride)
     int compact;
     // mode
     int forcing;       // 0 EDM, 1 SHIFT
