@@ -53,6 +53,7 @@ struct lbm {
     int nbsolid;
     int nfluid;       // fluid cells (masked domains)
     bool use_list;    // hot kernels iterate over the fluid-cell list (porous domains)
+    bool has_bmask;   // fluid-neighbour masks of the boundary solids are stored behind their list
     bool compact_on;  // lbm_step keeps the populations in fluid-list order (lbm_compact.cuh)
     bool is_compact;  // layout of the current population buffer
     long long nbr_stride;
@@ -323,6 +324,28 @@ __global__ void k_list_boundary_solids(Geo g, const uint32_t* __restrict__ flags
     if (any) list[atomicAdd(counter, 1)] = id;
 }
 
+// per boundary solid: which neighbours are fluid (same wrap/clamp indexing), so that K1b does not gather 18 flag words
+template <class L>
+__global__ void k_bsolid_masks(Geo g, int nb, const uint32_t* __restrict__ flags, const int* __restrict__ list, uint32_t* __restrict__ bmask) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nb) return;
+    const int id = list[b];
+    const int x = id % g.nx, t = id / g.nx, y = t % g.ny, z = t / g.ny;
+    const int n[3] = {g.nx, g.ny, g.nz};
+    uint32_t m = 0;
+    static_for<1, L::Q>([&](auto I) {
+        constexpr int i = I;
+        int pc[3] = {x + L::E[i][0], y + L::E[i][1], z + L::E[i][2]};
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (pc[a] < 0) pc[a] = g.periodic[a] ? pc[a] + n[a] : 0;
+            if (pc[a] >= n[a]) pc[a] = g.periodic[a] ? pc[a] - n[a] : n[a] - 1;
+        }
+        if (!(flags[pc[0] + g.nx * (pc[1] + g.ny * pc[2])] & SOLID_BIT)) m |= 1u << i;
+    });
+    bmask[b] = m;
+}
+
 // Fluid-cell list in ascending order (stream compaction in three small kernels: per-block counts, scan, fill).
 constexpr int COMPACT_BLOCK = 1024;
 __global__ void __launch_bounds__(COMPACT_BLOCK) k_fluid_count(int N, const uint32_t* __restrict__ flags, int* __restrict__ blockcnt,
@@ -542,6 +565,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
         p.f_in = h->ws + h->cv.f[in_buf];
         p.f_out = h->ws + h->cv.f[out_buf];
         p.nbsolid = h->nbsolid;
+        p.bmask = h->has_bmask ? reinterpret_cast<const uint32_t*>(h->ws + h->cv.bsolid) + h->nbsolid : nullptr;
         p.nfluid = h->nfluid;
         p.nbr_stride = h->nbr_stride;
         p.cplane = h->nbr_stride;
@@ -647,6 +671,7 @@ int prepare(lbm* h) {
     h->nbsolid = 0;
     h->nfluid = h->N;
     h->use_list = false;
+    h->has_bmask = false;
     CU(cudaMemsetAsync(h->ws + h->cv.psi, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
     CU(cudaMemsetAsync(h->ws + h->cv.rho, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
     if (h->bnd) {
@@ -694,6 +719,15 @@ int prepare(lbm* h) {
                 CU(cudaGetLastError());
                 h->launches += 4;
                 CU(cudaMemsetAsync(h->ws + h->cv.rho, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
+                // fluid-neighbour masks behind the list (the region holds N entries)
+                h->has_bmask = 2LL * h->nbsolid <= h->N;
+                if (h->has_bmask) {
+                    uint32_t* bm = reinterpret_cast<uint32_t*>(list + h->nbsolid);
+                    if (h->d == 2) k_bsolid_masks<D2Q9><<<(h->nbsolid + 255) / 256, 256, 0, h->stream>>>(g, h->nbsolid, flags, list, bm);
+                    else k_bsolid_masks<D3Q19><<<(h->nbsolid + 255) / 256, 256, 0, h->stream>>>(g, h->nbsolid, flags, list, bm);
+                    CU(cudaGetLastError());
+                    h->launches++;
+                }
             }
             // with most cells solid the dense mapping wastes lanes and issue slots on them: one thread per fluid cell
             h->use_list = h->nfluid < h->N / 2;
@@ -866,6 +900,7 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->force_rho = false;
     h->nbsolid = 0;
     h->nfluid = h->N;
+    h->has_bmask = false;
     h->compact_on = false;
     h->is_compact = false;
     h->nbr_stride = 0;

@@ -133,6 +133,7 @@ struct KParams {
     const uint32_t* flags;  // [N] (only read when BND)
     const int* bsolid; // boundary-solid list
     int nbsolid;
+    const uint32_t* bmask;  // per boundary solid: bit i <=> the neighbour at x + e_i is fluid (NULL: test the flags)
     const int* flist;  // fluid-cell list, ascending (list mode of the hot kernels on porous domains)
     int nfluid;
     // compact mode (lbm_compact.cuh): neighbour table [(Q-1)][nbr_stride] of extended indices; psi in extended order
@@ -329,11 +330,12 @@ __global__ void __launch_bounds__(128) k_virtual_density(const __grid_constant__
     CT num[NC], den = CT(0);
 #pragma unroll
     for (int k = 0; k < NC; ++k) num[k] = CT(0);
+    const uint32_t fm = p.bmask ? __ldg(p.bmask + b) : 0u;
     static_for<1, L::Q>([&](auto I) {
         constexpr int i = I;
         constexpr CT w = CT(L::WN[i]) / CT(L::WD);
         const int nb = id + nbr_offset<L::E[i][0], L::E[i][1], L::E[i][2]>(c);
-        if (!(__ldg(p.flags + nb) & SOLID_BIT)) {
+        if (p.bmask ? ((fm >> i) & 1u) != 0u : !(__ldg(p.flags + nb) & SOLID_BIT)) {
             den += w;
 #pragma unroll
             for (int k = 0; k < NC; ++k) num[k] += w * p.rho[(long long)k * p.N + nb];
