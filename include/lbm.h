@@ -159,7 +159,11 @@ LBM_API int lbm_set_face_bc(lbm_t* h, int face, int kind, const double* rho_w, c
  * element type of the arrays. */
 LBM_API int lbm_init_fields(lbm_t* h, const void* const* rho, const void* u, int dtype, int on_device);
 
-/* Enqueue n >= 0 time steps (S1..S7) on the stream.  Asynchronous; no host synchronisation. */
+/* Enqueue n >= 0 time steps (S1..S7) on the stream.  Asynchronous; no host synchronisation.
+ * Layout note: on a masked domain with at most a quarter of the cells fluid (and a plain Shan-Chen force) the steps
+ * run on a fluid-compact copy of the populations (lbm_hot_path reports LBM_PATH_TWO_PASS_COMPACT); the first step
+ * after, and the first export / import after such steps, each cost one extra copy kernel.  Results are bit-identical
+ * to the dense layout; solid cells read back as f_eq(1,0), whatever lbm_set_populations had put there. */
 LBM_API int lbm_step(lbm_t* h, int n);
 
 /* S8: rho^k (virtual density at boundary solids, 0 inside solids), u = (sum_k j^k + 1/2 sum_k F^k)/sum_k rho^k
