@@ -53,6 +53,7 @@ struct lbm {
     int nbsolid;
     int nfluid;       // fluid cells (masked domains)
     bool use_list;    // hot kernels iterate over the fluid-cell list (porous domains)
+    bool pdl;         // lbm_step on a small domain: hot kernels are launched as programmatic dependents
     bool has_bmask;   // fluid-neighbour masks of the boundary solids are stored behind their list
     bool compact_on;  // lbm_step keeps the populations in fluid-list order (lbm_compact.cuh)
     bool is_compact;  // layout of the current population buffer
@@ -549,6 +550,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.variant = h->fvariant;
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;
     a.pfd = 0;
+    a.pdl = h->pdl ? 1 : 0;
     a.used_kernel = op == OP_FUSED ? &h->last_path : nullptr;
     if (const char* e = std::getenv("LBM_TUNE_FUSED_PFD")) a.pfd = std::atoi(e);
     a.stream = h->stream;
@@ -900,6 +902,7 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->force_rho = false;
     h->nbsolid = 0;
     h->nfluid = h->N;
+    h->pdl = false;
     h->has_bmask = false;
     h->compact_on = false;
     h->is_compact = false;
@@ -1040,6 +1043,10 @@ int lbm_step(lbm_t* h, int n) {
     // be captured (the legacy default stream): then, and for large domains, the kernels are launched one by one.
     constexpr int GRAPH_STEPS = 16;   // even: the ping-pong parity is the same after a replay
     const bool small = (long long)h->N * h->cfg.n_components <= (1LL << 22);
+    // ... and each kernel is launched as a programmatic dependent of the one before it (pdl_begin), which hides most of
+    // the launch latency between them
+    struct PdlScope { lbm* h; ~PdlScope() { h->pdl = false; } } pdl_scope{h};
+    h->pdl = small && !h->profiling && !std::getenv("LBM_TUNE_NO_PDL");
     if (small && !h->profiling && !h->gfailed && n >= 2 * GRAPH_STEPS + 1 && !std::getenv("LBM_TUNE_NO_GRAPH")) {
         if ((rc = step_once())) return rc;      // first step plainly: one-time kernel attribute set-up happens outside capture
         --n;

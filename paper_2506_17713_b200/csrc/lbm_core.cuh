@@ -177,6 +177,15 @@ struct FieldIO {
     int c0, cnt;
 };
 
+// Programmatic dependent launch (small, launch-bound domains: lbm_launch.cuh launches the hot kernels with the
+// programmatic-serialisation attribute): let the next kernel's CTAs be scheduled right away, then wait until the previous
+// kernel has completed and its writes are visible.  Every hot kernel calls this before it touches global memory, so the
+// chain stays ordered; without the launch attribute both instructions do nothing.
+__device__ __forceinline__ void pdl_begin() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // ------------------------------------------------------------------ storage conversion
 template <class CT, class ST> struct Conv;
 template <> struct Conv<float, float> {
@@ -323,6 +332,7 @@ __device__ __forceinline__ CT feq(CT r, const CT (&u)[3], CT uu15) {
 // ------------------------------------------------------------------ K1b: virtual density at boundary solids
 template <class L, int NC, class CT>
 __global__ void __launch_bounds__(128) k_virtual_density(const __grid_constant__ KParams<CT> p) {
+    pdl_begin();
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= p.nbsolid) return;
     const int id = __ldg(p.bsolid + b);

@@ -545,6 +545,7 @@ __device__ __forceinline__ void apply_face_rules(const KParams<CT>& p, const Cel
 template <class L, int NC, class CT, class ST, bool BND, int VEC, bool LIST = false>
 __global__ void __launch_bounds__(256, (VEC == 1 ? 4 : 1)) k_moments_v(const __grid_constant__ KParams<CT> p) {
     static_assert(!LIST || (BND && VEC == 1), "list mode is one cell per thread on a masked domain");
+    pdl_begin();
     unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
     if constexpr (LIST) {
         if (vid >= (unsigned)p.nfluid) return;
@@ -579,6 +580,7 @@ template <class L, int NC, class CT, class ST, int COLL, bool BND, int VEC, bool
 __global__ void __launch_bounds__(128, ((LIST && sizeof(ST) == 2) ? 6 : 1)) k_step_v(const __grid_constant__ KParams<CT> p) {
     static_assert(!LIST || (BND && VEC == 1), "list mode is one cell per thread on a masked domain");
     static_assert(!ZC || (VEC == 1 && !LIST && COLL != 2), "the Zhang-Chen variant is one cell per thread");
+    pdl_begin();
     unsigned vid = blockIdx.x * blockDim.x + threadIdx.x;
     if constexpr (LIST) {
         if (vid >= (unsigned)p.nfluid) return;

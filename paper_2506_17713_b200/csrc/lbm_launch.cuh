@@ -31,6 +31,7 @@ struct LaunchArgs {
     int pfd;             // OP_FUSED (warp-specialised): L2 prefetch distance in planes
     int* used_kernel;    // OP_FUSED, out: 1 = lock-step k_fused_v ran, 2 = warp-specialised k_fused_ws
     int wref;            // OP_FUSED: rho_ref != 0 (populations stored shifted by w_i rho_ref)
+    int pdl;             // OP_MOMENTS / OP_VIRTUAL / OP_STEP (dense mapping): programmatic dependent launch (pdl_begin)
     cudaStream_t stream;
 };
 
@@ -84,6 +85,23 @@ cudaError_t launch(const LaunchArgs& a) {
         if (a.bnd) fn(IC<1>{});
         else fn(IC<0>{});
     };
+    // hot kernels of the dense mapping: plain launch, or with the programmatic-serialisation attribute (pdl_begin)
+    auto launch_hot = [&](auto kernel, dim3 g, unsigned block) {
+        if (!a.pdl) {
+            kernel<<<g, block, 0, a.stream>>>(p);
+            return;
+        }
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = g;
+        cfg.blockDim = dim3(block);
+        cfg.stream = a.stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, kernel, p);
+    };
     switch (a.op) {
         case OP_MOMENTS:
             with_nc([&](auto NC) {
@@ -100,15 +118,15 @@ cudaError_t launch(const LaunchArgs& a) {
                         }
                     }
                     if (a.vec == VW && VW > 1)
-                        k_moments_v<L, NC, CT, ST, (B != 0), VW><<<grid(p.N / VW, 256), 256, 0, a.stream>>>(p);
+                        launch_hot(k_moments_v<L, NC, CT, ST, (B != 0), VW>, grid(p.N / VW, 256), 256);
                     else
-                        k_moments_v<L, NC, CT, ST, (B != 0), 1><<<grid(p.N, 256), 256, 0, a.stream>>>(p);
+                        launch_hot(k_moments_v<L, NC, CT, ST, (B != 0), 1>, grid(p.N, 256), 256);
                 });
             });
             break;
         case OP_VIRTUAL:
             if (p.nbsolid > 0)
-                with_nc([&](auto NC) { k_virtual_density<L, NC, CT><<<grid(p.nbsolid, 128), 128, 0, a.stream>>>(p); });
+                with_nc([&](auto NC) { launch_hot(k_virtual_density<L, NC, CT>, grid(p.nbsolid, 128), 128); });
             break;
         case OP_STEP:
             with_nc([&](auto NC) {
@@ -137,9 +155,9 @@ cudaError_t launch(const LaunchArgs& a) {
                             }
                         }
                         if (a.vec == VW && VW > 1)
-                            k_step_v<L, NC, CT, ST, C_, (B != 0), VW><<<grid(p.N / VW, 128), 128, 0, a.stream>>>(p);
+                            launch_hot(k_step_v<L, NC, CT, ST, C_, (B != 0), VW>, grid(p.N / VW, 128), 128);
                         else
-                            k_step_v<L, NC, CT, ST, C_, (B != 0), 1><<<grid(p.N, 128), 128, 0, a.stream>>>(p);
+                            launch_hot(k_step_v<L, NC, CT, ST, C_, (B != 0), 1>, grid(p.N, 128), 128);
                     });
                 });
             });
