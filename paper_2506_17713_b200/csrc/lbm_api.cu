@@ -732,8 +732,8 @@ int prepare(lbm* h) {
                 }
             }
             // with most cells solid the dense mapping wastes lanes and issue slots on them: one thread per fluid cell
-            h->use_list = h->nfluid < h->N / 2;
-            if (const char* e = std::getenv("LBM_TUNE_LIST")) h->use_list = std::atoi(e) != 0;
+            h->use_list = h->nfluid > 0 && h->nfluid < h->N / 2;   // (an all-solid domain has nothing to list)
+            if (const char* e = std::getenv("LBM_TUNE_LIST")) h->use_list = h->nfluid > 0 && std::atoi(e) != 0;
         }
     }
     h->dirty = false;

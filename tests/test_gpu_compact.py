@@ -104,3 +104,23 @@ def test_compact_d2q9_channels_and_pure_streaming():
     assert g.hot_path == "two_pass_compact"
     for k in range(2):
         assert np.array_equal(o.get_populations(k)[:, fl], g.get_populations(k)[:, fl])
+
+
+def test_degenerate_masks_all_solid_and_single_fluid_cell():
+    """nothing to update, and one fluid cell whose every link bounces back: mass stays put"""
+    from paper_2506_17713_b200 import binding
+    wl, inp = W.config5(16, "f64")
+    e, w, opp = binding.get_lattice("D3Q19")
+    N = 16 ** 3
+    g = make_gpu(wl, dict(inp, mask=np.ones(N, np.uint8)))
+    g.step(3)
+    assert np.abs(g.get_populations(0) - np.asarray(w)[:, None]).max() <= 1e-15
+    mask = np.ones(N, np.uint8)
+    mask[5 + 16 * (6 + 16 * 7)] = 0
+    inp1 = dict(inp, mask=mask)
+    o, g = make_oracle(wl, inp1), make_gpu(wl, inp1)
+    o.step(5); g.step(5)
+    assert g.hot_path == "two_pass_compact"
+    fl = mask == 0
+    assert np.abs(o.get_populations(0)[:, fl] - g.get_populations(0)[:, fl]).max() <= TOL64
+    assert abs(g.get_populations(0)[:, fl].sum() - np.asarray(inp["rho"][0])[fl].sum()) <= 1e-13
