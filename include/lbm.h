@@ -120,8 +120,14 @@ typedef struct {
     lbm_eos_t eos[2];
     double G[2][2];          /* g_kk' of Eq. 13; Green's function weights are w_i/c_s^2 (reading R2) */
     lbm_wetting_t wet[2];
-    double tau[2];           /* BGK relaxation time; with MRT = 1/s_nu (enters the common velocity and LBM_SHIFT) */
-    double mrt_rates[2][19]; /* diagonal of S in the moment order of DESIGN.md R9 (first q entries used) */
+    double tau[2];           /* BGK relaxation time (> 1/2).  It is also the relaxation time of the momentum that enters the
+                                common velocity u' = sum_k (j^k/tau_k) / sum_k (rho^k/tau_k) (R6) and LBM_SHIFT (R7).
+                                With LBM_MRT the rates below decide everything and tau is not read. */
+    double mrt_rates[2][19]; /* diagonal of S in the moment order of DESIGN.md R9 (first q entries used).  The momentum rows
+                                (3, 5 and, on D3Q19, 7) must share one non-zero rate s_j (LBM_E_INVALID otherwise): 1/s_j
+                                takes the place of tau_k in the common velocity and in LBM_SHIFT, so that a collision
+                                changes the total momentum by exactly sum_k F^k (Eq. 3 + Eq. 10)
+                                whatever the other rates are. */
     double rho_ref;          /* populations are stored as f_i - w_i*rho_ref (reading R16); 0 = plain */
     double zc_A[2];          /* A_kk of Eq. 11 / 13: F^k = A_kk F_ZC^k + (1 - A_kk) F_SC^k with the Zhang-Chen
                                 force F_ZC^k = -sum_i G_i U^k(x+e_i) e_i, U^k = alpha p_EOS - c_s^2 rho (Eq. 12).  0 = plain

@@ -25,11 +25,17 @@
 //   A-weighted Zhang-Chen force (Eq. 11-13): F_ZC = -grad U against
 //   a re-typed EOS, weighted sum, coexistence -> Maxwell with A ~ -0.19,
 //   mass / momentum conservation.
-//   Surface-tension control (Eq. 14-16, D2Q9 MRT): sigma(kappa) / sigma(0)
-//   = 1 - kappa within 0.04 at kappa = 0.5 with the coexistence densities kept.
-//   PARITY UNPINNED: the O(u^2) terms of the pressure-face (anti-bounce-back)
-//   formula -- reading R10 -- have no paper value or closed form to be held to;
-//   see DESIGN.md.
+//   Surface-tension control (Eq. 14-16, D2Q9 MRT): domain-summed moments after one
+//   step = C of Eq. 15 with Q of Eq. 16 (incl. the A_kk term) evaluated by hand; sigma(kappa = 0.5)
+//   / sigma(0) against the ratio of the paper's Table 2 (CS row: 0.457).
+//   Single terms (tests/test_oracle_terms.py): velocity shift at tau != 1 and MRT (momentum gain per
+//   step = total force, exactly), the w_i weights of rho_ave in Eq. 17 on a hand-built non-uniform
+//   neighbourhood, Eq. 6's half force (u = (t + 1/2) a), D3Q19 MRT rate <-> row assignment (shear
+//   waves on axes and face diagonals), and the O(u^2) bracket of the pressure face (a uniform
+//   equilibrium flow at any Mach number is an exact fixed point between two pressure faces).
+//   Contact angles of configs 2 and 4 (60 / 40 deg) from a circle fit of the meniscus.
+//   PARITY UNPINNED: nothing on the step itself.  (Table 2's absolute surface tensions and the
+//   Fig. 4-8 curves depend on unpublished alpha, A, kappa and are not reproduced.)
 //
 // State = post-stream populations f_i^k(x,t) (in the storage dtype, possibly
 // shifted by w_i*rho_ref, reading R16).  One step = S1..S7 below.
@@ -97,7 +103,7 @@ struct olbm_config {
     double rho0[2];            // SC93 psi = rho0 (1 - exp(-rho/rho0))
     double G[2][2];            // g_kk' of Eq. 13, weights w_i/c_s^2 (R2)
     double wet_phi[2], wet_drho[2], wet_lo[2], wet_hi[2];  // Eq. 17 + limiter
-    double tau[2];             // BGK tau; for MRT = 1/s_nu (used in S5 and shift forcing)
+    double tau[2];             // BGK tau (MRT: the rates below decide; tau is not read)
     double mrt_rates[2][19];   // diagonal of S, moment order of R9
     double rho_ref;            // storage shift: stored = f_i - w_i*rho_ref (R16)
     double zc_A[2];            // A_kk of Eq. 11/13: F^k = A_kk F_ZC^k + (1 - A_kk) F_SC^k; 0 = pure Shan-Chen
@@ -391,6 +397,14 @@ struct Sim : SimBase {
         return 0;
     }
 
+    // Relaxation time of the momentum of component k: tau_k for BGK; for MRT 1 / (rate of the momentum rows), which
+    // need not be 1/s_nu.  It is this time that enters the common velocity (R6) and the velocity shift (R7):
+    // only then does a collision change the total momentum by exactly sum_k F^k (Eq. 3 + Eq. 10).
+    T momentum_time(int k) const {
+        if (c.collision == COLL_MRT) return T(1) / (T)c.mrt_rates[k][3];
+        return (T)c.tau[k];
+    }
+
     // ---- f_eq (R1): w_i rho [1 + e.u/cs2 + (e.u)^2/(2 cs2^2) - u.u/(2 cs2)]
     T feq(int i, T r, const T* u) const {
         T eu = T(0), uu = T(0);
@@ -537,6 +551,7 @@ struct Sim : SimBase {
             }
         }
         // S5 (R6): common velocity u' = sum_k (j^k/tau_k) / sum_k (rho^k/tau_k); = j/rho for one component
+        // (tau_k = momentum_time(k))
 #pragma omp parallel for schedule(static) if (N >= 262144)
         for (int64_t id = 0; id < N; ++id) {
             if (solid[id]) { for (int a = 0; a < 3; ++a) ucom[a][id] = T(0); continue; }
@@ -545,8 +560,8 @@ struct Sim : SimBase {
             } else {
                 T den = T(0), num[3] = {T(0), T(0), T(0)};
                 for (int k = 0; k < nc; ++k) {
-                    den += rho[k][id] / (T)c.tau[k];
-                    for (int a = 0; a < 3; ++a) num[a] += j[k][a][id] / (T)c.tau[k];
+                    den += rho[k][id] / momentum_time(k);
+                    for (int a = 0; a < 3; ++a) num[a] += j[k][a][id] / momentum_time(k);
                 }
                 for (int a = 0; a < 3; ++a) ucom[a][id] = num[a] / den;
             }
@@ -573,7 +588,7 @@ struct Sim : SimBase {
                 for (int a = 0; a < 3; ++a) du[a] = F[k][a][id] / r;
                 T ueq[3] = {u[0], u[1], u[2]};
                 if (c.forcing == FORCE_SHIFT)  // R7: u_eq = u' + tau F/rho, no source term
-                    for (int a = 0; a < 3; ++a) ueq[a] = u[a] + tau * du[a];
+                    for (int a = 0; a < 3; ++a) ueq[a] = u[a] + momentum_time(k) * du[a];
                 for (int i = 0; i < q; ++i) fe[i] = feq(i, r, ueq);
                 if (c.collision == COLL_BGK) {
                     // Eq. 3 line 1
@@ -778,6 +793,12 @@ bool config_ok(const olbm_config& c) {
         if (c.psi_kind[k] < 0 || c.psi_kind[k] > PSI_SC93) return false;
         if (c.psi_kind[k] <= PSI_EOS_RKS && !(c.G[k][k] < 0.0)) return false;  // R4: g_kk < 0 under the root
         if (!(c.tau[k] > 0.5)) return false;
+        if (c.collision == COLL_MRT) {   // the momentum rows share one non-zero rate (momentum_time)
+            const int nj = c.lattice == LAT_D2Q9 ? 2 : 3;
+            if (!(c.mrt_rates[k][3] > 0.0)) return false;
+            for (int a = 1; a < nj; ++a)
+                if (c.mrt_rates[k][3 + 2 * a] != c.mrt_rates[k][3]) return false;
+        }
     }
     return true;
 }

@@ -103,6 +103,12 @@ int check_config(const lbm_config_t* c) {
         if (c->zc_A[k] != 0.0 && e.psi_kind > LBM_PSI_EOS_RKS) return LBM_E_INVALID;   // U of Eq. 12 needs an EOS
         if (c->st_kappa[k] != 0.0 && (c->lattice != LBM_D2Q9 || c->collision != LBM_MRT)) return LBM_E_UNSUPPORTED;
         if (!(c->tau[k] > 0.5)) return LBM_E_INVALID;
+        if (c->collision == LBM_MRT) {   // the momentum rows share one non-zero rate (lbm.h: mrt_rates)
+            const int nj = c->lattice == LBM_D2Q9 ? 2 : 3;
+            if (!(c->mrt_rates[k][3] > 0.0)) return LBM_E_INVALID;
+            for (int a = 1; a < nj; ++a)
+                if (c->mrt_rates[k][3 + 2 * a] != c->mrt_rates[k][3]) return LBM_E_INVALID;
+        }
     }
     return LBM_OK;
 }
@@ -201,8 +207,11 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
     else lattice_weights<D3Q19>(w);
     for (int i = 0; i < h->q; ++i) p.wref[i] = (CT)(w[i] * c.rho_ref);
     for (int k = 0; k < c.n_components; ++k) {
-        p.tau[k] = (CT)c.tau[k];
-        p.inv_tau[k] = (CT)(1.0 / c.tau[k]);
+        // relaxation time of the momentum (common velocity R6, velocity shift R7): tau for BGK, 1 / (rate of the
+        // momentum rows) for MRT -- only then does a collision change the total momentum by exactly sum_k F^k
+        const double tmom = c.collision == LBM_MRT ? 1.0 / c.mrt_rates[k][3] : c.tau[k];
+        p.tau[k] = (CT)tmom;
+        p.inv_tau[k] = (CT)(1.0 / tmom);
         for (int kp = 0; kp < c.n_components; ++kp) p.G[k][kp] = (CT)c.G[k][kp];
         // BGK as one linear combination (lbm_hot.cuh collide): EDM  f* = (1-w) f + (w-1) feq(u') + feq(u'+du),
         // SHIFT  f* = (1-w) f + w feq(u' + tau du), w = 1/tau

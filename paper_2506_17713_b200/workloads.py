@@ -30,6 +30,13 @@ PR_T_07 = 0.05104540285          # 0.7 * T_c, T_c = 0.0778 a/(0.45724 b R)
 PR_RHO_V_07 = 0.0556351
 PR_RHO_L_07 = 8.0803216
 
+# Wetting parameters of configs 2 and 4 (Eq. 17, second branch): Delta rho of the NON-wetting component at the wall.
+# The contact angle has no closed form in (phi, Delta rho): calibrated with the oracle on a flat-walled
+# channel (circle fit of the meniscus, tests/test_oracle_physics.py::test_contact_angles_of_configs_2_and_4) --
+# 0.32 -> 60 +- 2 deg (config 2), 0.60 -> 40 +- 2 deg (config 4); sweep in DESIGN.md section 4.
+C2_DRHO_B = 0.32
+C4_DRHO_NW = 0.60
+
 # MRT relaxation rates (reading R9): conserved rows 1.0, s_nu = 1/tau
 def mrt_rates(lattice: str, tau: float = 1.0):
     s_nu = 1.0 / tau
@@ -84,7 +91,7 @@ def config1(n: int = 64, dtype: str = "f64"):
 
 
 # ---------------------------------------------------------------- config 2
-def config2(nx: int = 512, ny: int = 256, dtype: str = "f32", wall: int = 8, drho_b: float = 0.30):
+def config2(nx: int = 512, ny: int = 256, dtype: str = "f32", wall: int = 8, drho_b: float = C2_DRHO_B):
     """D2Q9 two components between two solid plates (capillary geometry), SC93 psi, G_AB = 3.5 classic."""
     g_ab = 3.5 / 3.0  # classic SC93 G = 3.5 with weights w_i  ==  g = 3.5*c_s^2 with weights w_i/c_s^2 (R15)
     wl = dict(
@@ -182,7 +189,7 @@ def sphere_pack_mask(nx, ny, nz, porosity=0.20, rmin=6.0, rmax=14.0, buffer=8, s
     return solid.astype(np.uint8).reshape(-1), por
 
 
-def config4(n: int = 400, store_dtype: str = "f16", drho_nw: float = 0.5, buffer: int = 8):
+def config4(n: int = 400, store_dtype: str = "f16", drho_nw: float = C4_DRHO_NW, buffer: int = 8):
     """D3Q19 two components in a seeded sphere pack; velocity inlet x=0 (non-wetting), pressure outlet x=n-1."""
     g_ab = 3.5 / 3.0
     buffer = min(buffer, max(2, n // 8))

@@ -7,6 +7,8 @@ on the same seeded inputs.  Gates (BASELINE.json north_star):
     (DESIGN.md "Tolerances")
 Sizes span several thread blocks and have ragged tails (nx not a multiple of the block size).
 """
+from pathlib import Path
+
 import numpy as np
 import pytest
 
@@ -120,6 +122,10 @@ def test_config3_mrt_peng_robinson():
     f32o = [o32.get_populations(0)]
     d_gpu = np.abs(fg[0] - fo[0]).max() / np.abs(fo[0]).max()
     d_cpu = np.abs(f32o[0] - fo[0]).max() / np.abs(fo[0]).max()
+    print(f"config 3 fp32 after 100 steps, relative to the fp64 oracle: gpu {d_gpu:.3e}, fp32 oracle {d_cpu:.3e}")
+    (Path(__file__).resolve().parent.parent / "gpurun_out").mkdir(exist_ok=True)
+    (Path(__file__).resolve().parent.parent / "gpurun_out" / "config3_fp32_distance.txt").write_text(
+        f"d_gpu {d_gpu:.6e}\nd_cpu {d_cpu:.6e}\n")
     assert d_gpu <= max(TOL32, 3 * d_cpu), (d_gpu, d_cpu)
 
 
@@ -188,11 +194,8 @@ def test_collision_and_forcing_variants(lattice, n, collision, forcing):
               psi_kind=["CS"], eos=[dict(a=W.CS_A, b=W.CS_B, R=W.CS_R, T=W.CS_T_085)], G=[[-1.0]],
               collision=collision, tau=[tau], forcing=forcing, compute_dtype="f64", store_dtype="f64")
     if collision == "MRT":
-        rates = W.mrt_rates(lattice, tau)
-        if forcing == "SHIFT":   # momentum rows must relax at s_nu for the shifted equilibrium to inject F
-            for r in ([3, 5] if lattice == "D2Q9" else [3, 5, 7]):
-                rates[r] = 1.0 / tau
-        wl["mrt_rates"] = [rates]
+        # momentum rows at rate 1, s_nu = 1/tau: the shift uses the momentum rows' own relaxation time (R7)
+        wl["mrt_rates"] = [W.mrt_rates(lattice, tau)]
     inp = small_inputs(wl, 5, 0.1, 0.2)
     o, g, fo, fg = run_pair(wl, inp, 100)
     assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
@@ -328,10 +331,19 @@ def test_coexistence_densities_match_oracle(dtype):
     rg = g.get_macroscopic()[0][0].reshape(ny, nx)[0]
     assert abs(rg[nx // 2] - ro[nx // 2]) <= 1e-4
     assert abs(rg[0] - ro[0]) <= 1e-4
-    # mass: every stored population is rounded once per step, so the drift is bounded by steps * eps/2
-    # relative (fp32: 6000 * 2^-24 = 3.6e-4; observed ~5e-5), fp64: 6000 * 2^-53 = 7e-13
+    # mass: fp64 to 1e-11.  fp32 rounds every stored population once per step and sum_i f_eq,i = rho only holds to
+    # rounding, which drifts systematically (the fp32 ORACLE itself drifts by 4.5e-5 relative over these 6000 steps):
+    # the CUDA path may drift at most twice as far as the fp32 oracle does on the same run.
     m0 = rho0.sum()
-    assert abs(g.get_populations(0).sum() - m0) <= (1e-11 if dtype == "f64" else 6000 * 2.0 ** -24) * m0
+    d_gpu = abs(g.get_populations(0).sum() - m0) / m0
+    if dtype == "f64":
+        assert d_gpu <= 1e-11
+    else:
+        o32 = make_oracle(wl, inp)
+        o32.step(6000)
+        d_cpu = abs(o32.get_populations(0).sum() - m0) / m0
+        print(f"fp32 mass drift over 6000 steps: gpu {d_gpu:.3e}, fp32 oracle {d_cpu:.3e}")
+        assert d_gpu <= 2 * d_cpu, (d_gpu, d_cpu)
 
 
 # ------------------------------------------------------------------ API behaviour

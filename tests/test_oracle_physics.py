@@ -122,7 +122,9 @@ def test_laplace_law():
     assert np.abs(sig / sig.mean() - 1).max() < 0.03
 
 
-def _meniscus_offset(drho_b, nx=64, ny=26, wall=2, steps=4000):
+def _meniscus(drho_b, nx=64, ny=26, wall=2, steps=4000):
+    """Slug of component A between two flat plates (the wetting set-up of configs 2 and 4: SC93 psi, g_AB = 7/6,
+    Delta rho on the other component B); returns a function row -> x of the right-hand A|B interface."""
     g = 3.5 / 3
     wl = base_wl("D2Q9", (nx, ny, 1), nc=2, psi_kind=["SC93"] * 2, eos=[dict(rho0=1.0)] * 2, G=[[0, g], [g, 0]],
                  wetting=[dict(phi=1, drho=0, lo=0, hi=1.2), dict(phi=1, drho=drho_b, lo=0, hi=1.2)])
@@ -147,6 +149,28 @@ def _meniscus_offset(drho_b, nx=64, ny=26, wall=2, steps=4000):
                 return i + d[i] / (d[i] - d[i + 1])
         raise AssertionError("no interface")
 
+    return cross
+
+
+def _contact_angle_circle_fit(drho_b, nx=64, ny=32, wall=2, steps=6000, skip=3):
+    """Contact angle of component A from a least-squares circle through the interface points of all fluid rows but the
+    `skip` next to each wall (centre on the channel axis): cos(theta) = (H/2) / R, H = plate distance (the walls sit
+    half a cell outside the first / last fluid row)."""
+    cross = _meniscus(drho_b, nx, ny, wall, steps)
+    rows = np.arange(wall + skip, ny - wall - skip)
+    xs = np.array([cross(int(r)) for r in rows])
+    if np.ptp(xs) < 0.05:
+        return 90.0
+    yy = (rows - (ny - 1) / 2.0) ** 2
+    # (x - xc)^2 + yy = R^2  ->  x^2 + yy = 2 xc x + (R^2 - xc^2)
+    (xc, cc), *_ = np.linalg.lstsq(np.stack([2 * xs, np.ones_like(xs)], axis=1), xs ** 2 + yy, rcond=None)
+    R = np.sqrt(cc + xc * xc)
+    t = np.degrees(np.arccos(min(1.0, (ny - 2 * wall) / 2.0 / R)))
+    return t if xs[len(xs) // 2] < xc else 180.0 - t      # centre of curvature on the B side: A wets
+
+
+def _meniscus_offset(drho_b, nx=64, ny=26, wall=2, steps=4000):
+    cross = _meniscus(drho_b, nx, ny, wall, steps)
     H = ny - 2 * wall
     dx = cross(wall) - cross(ny // 2)   # > 0: component A creeps along the wall (A wets)
     # circular meniscus: dx = (H/2)(1 - sin t)/cos t between the wall and the centre line
@@ -165,6 +189,20 @@ def test_contact_angle_neutral_and_monotone():
     dx2, t2 = _meniscus_offset(0.30)
     assert 0 < dx1 < dx2
     assert angle > t1 > t2 > 30.0
+
+
+def test_contact_angles_of_configs_2_and_4():
+    """BASELINE.json: config 2 "wall virtual density set for a 60 deg contact angle", config 4 "a 40 deg contact angle for
+    the wetting phase".  The Delta rho values workloads.py gives the two configs produce these angles (within 4 deg, the
+    accuracy of a circle fit through a 3-cell-wide interface in a 28-cell channel).  Config 4 runs D3Q19; its
+    z-invariant solutions are D2Q9 solutions (the D3Q19 weights project onto the D2Q9 ones: 1/18 + 2/36 = 1/9,
+    1/3 + 2/18 = 4/9), so the flat-wall calibration is done in 2-D."""
+    assert abs(_contact_angle_circle_fit(W.C2_DRHO_B) - 60.0) < 4.0
+    assert abs(_contact_angle_circle_fit(W.C4_DRHO_NW) - 40.0) < 4.0
+    wl2, _ = W.config2(32, 16)
+    wl4, _ = W.config4(24)
+    assert wl2["wetting"][1]["drho"] == W.C2_DRHO_B and wl2["wetting"][0]["drho"] == 0.0
+    assert wl4["wetting"][0]["drho"] == W.C4_DRHO_NW and wl4["wetting"][1]["drho"] == 0.0
 
 
 # ------------------------------------------------------------------ NEXT-1: A-weighted Zhang-Chen force (Eq. 11-13)
