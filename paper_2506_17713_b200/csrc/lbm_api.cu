@@ -43,6 +43,8 @@ struct lbm {
     int fvariant;        // tuning variant of K2F (0 = default)
     int fmchunk;         // planes marched per CTA
     bool use_fused;      // decided in prepare()
+    bool eq_narrow;      // k_fused_eq tile: 32 x VEC/2 cells by 16 rows instead of 32 x VEC by 8
+    bool feq;            // one component, BGK, tau = 1: the collision result is f_eq(rho, u' + du) (k_fused_eq applies)
     int last_path;       // lbm_hot_path: what the last lbm_step ran
     // launch-bound (small) domains: GRAPH_STEPS time steps captured once into a CUDA graph and replayed
     cudaGraphExec_t gexec;
@@ -559,6 +561,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.variant = h->fvariant;
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;
     a.pfd = 0;
+    a.eq = h->feq ? (h->eq_narrow ? 2 : 1) : 0;
     a.pdl = h->pdl ? 1 : 0;
     a.used_kernel = op == OP_FUSED ? &h->last_path : nullptr;
     if (const char* e = std::getenv("LBM_TUNE_FUSED_PFD")) a.pfd = std::atoi(e);
@@ -629,6 +632,7 @@ FusedShape fused_shape_of(const lbm_config_t& c, int variant) {
 void plan_fused(lbm* h) {
     h->use_fused = false;
     const lbm_config_t& c = h->cfg;
+    h->feq = c.n_components == 1 && c.collision == LBM_BGK && c.tau[0] == 1.0 && !std::getenv("LBM_TUNE_NO_EQ");
     if (c.flags & (LBM_FLAG_TWO_PASS | LBM_FLAG_NO_COLLIDE)) return;
     if (c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0)))
         return;   // Zhang-Chen weight / surface-tension source: two-pass path
@@ -636,8 +640,10 @@ void plan_fused(lbm* h) {
     if ((unsigned long long)c.n_components * h->q * (unsigned long long)h->plane >= (1ULL << 32)) return;   // 32-bit element offsets
     if (h->d == 3 && c.nx % (16 / (int)h->sbytes) != 0 && h->fvariant == 0) h->fvariant = -1;   // k_fused_ws copies 16-byte pads
     const int nm = h->d == 3 ? c.nz : c.ny;
-    const int tx = h->fshape.wx * 32 * h->fshape.vec;
-    const long long tiles = (long long)((c.nx + tx - 1) / tx) * (h->d == 3 ? (c.ny + h->fshape.ty - 1) / h->fshape.ty : 1);
+    const bool eq_tile = h->feq && h->d == 3 && h->fvariant == 0;
+    const int tx = h->fshape.wx * 32 * h->fshape.vec / (eq_tile && h->eq_narrow ? 2 : 1);
+    const int ty = h->fshape.ty * (eq_tile && h->eq_narrow ? 2 : 1);
+    const long long tiles = (long long)((c.nx + tx - 1) / tx) * (h->d == 3 ? (c.ny + ty - 1) / ty : 1);
     // Chunks per column of tiles: every CTA pulls two extra planes and pays a few planes' worth of pipeline fill, and
     // CTAs run in waves of one per SM, so minimise  waves * (planes per chunk + 5)  (measured on 128^3 .. 512^3: the
     // model picks 16, 128 and 128 planes, the best of the sweeps in DESIGN.md 6)
@@ -898,6 +904,9 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     if (h->fshape.vec == 0 && h->fvariant != 0) { h->fvariant = 0; h->fshape = fused_shape_of(*cfg, 0); }
     h->fmchunk = 1;
     h->use_fused = false;
+    h->feq = false;
+    h->eq_narrow = false;
+    if (const char* e = std::getenv("LBM_TUNE_EQ_NARROW")) h->eq_narrow = std::atoi(e) != 0;
     h->last_path = LBM_PATH_NONE;
     h->gexec = nullptr;
     h->gcur = 0;

@@ -5,6 +5,7 @@
 #include <cstdlib>
 #include "lbm_fused.cuh"
 #include "lbm_fused_ws.cuh"
+#include "lbm_fused_eq.cuh"
 #include "lbm_compact.cuh"
 
 namespace lbmk {
@@ -29,7 +30,9 @@ struct LaunchArgs {
     int variant;         // OP_FUSED: 0 = default (warp-specialised k_fused_ws on D3Q19, lock-step k_fused_v on D2Q9);
                          //           -1 = lock-step kernel everywhere; 1.. = tuning experiments (LBM_FUSED_TUNING)
     int pfd;             // OP_FUSED (warp-specialised): L2 prefetch distance in planes
-    int* used_kernel;    // OP_FUSED, out: 1 = lock-step k_fused_v ran, 2 = warp-specialised k_fused_ws
+    int eq;              // OP_FUSED: one component, BGK, tau = 1 (f* is an equilibrium): the row-pipeline kernel k_fused_eq applies
+                         //           1 = wide tile (32 x VEC cells by 8 rows), 2 = narrow tile (32 x VEC/2 cells by 16 rows)
+    int* used_kernel;    // OP_FUSED, out: the lbm_path value of the kernel that ran
     int wref;            // OP_FUSED: rho_ref != 0 (populations stored shifted by w_i rho_ref)
     int pdl;             // OP_MOMENTS / OP_VIRTUAL / OP_STEP (dense mapping): programmatic dependent launch (pdl_begin)
     cudaStream_t stream;
@@ -253,8 +256,46 @@ cudaError_t launch(const LaunchArgs& a) {
                             done = true;
                         }
                     };
+                    // row-pipeline kernel (lbm_fused_eq.cuh): same tile, same opt-ins
+                    auto go_eq = [&](auto VEC, auto TY, auto WREF) {
+                        if constexpr (L::D == 3 && NC == 1 && C_ == 0) {
+                            using T = EqTile<L, CT, ST, VEC, TY>;
+                            auto kern = k_fused_eq<L, CT, ST, VEC, TY, (WREF != 0)>;
+                            static int ready[16] = {0};   // per device: 0 unknown, 1 usable, -1 not usable
+                            int dev = 0;
+                            cudaGetDevice(&dev);
+                            int& rd = ready[dev & 15];
+                            if (rd == 0) {
+                                cudaFuncAttributes fa;
+                                const cudaError_t e1 = cudaFuncGetAttributes(&fa, kern);
+                                // the register pool the kernel re-splits with setmaxnreg (a smaller one would make setmaxnreg.inc wait forever)
+                                const bool regs_ok = e1 == cudaSuccess &&
+                                                     fa.numRegs * T::THREADS >= T::REG_PROD * T::NPW * 32 + T::REG_CONS * T::NCW * 32;
+                                const cudaError_t e2 = regs_ok ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                                                      (int)T::SMEM) : cudaErrorUnknown;
+                                rd = (regs_ok && e2 == cudaSuccess) ? 1 : -1;
+                                cudaGetLastError();
+                            }
+                            if (rd < 0) return;
+                            dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + TY - 1) / TY),
+                                   (unsigned)((p.nz + a.i0 - 1) / a.i0));
+                            kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0);
+                            if (a.used_kernel) *a.used_kernel = 5;  // LBM_PATH_ONE_PASS_EQ
+                            done = true;
+                        }
+                    };
                     if constexpr (fs.vec > 0) {
                         if constexpr (L::D == 3) {
+                            if (a.variant == 0 && a.eq) {
+                                if (a.eq == 2) {
+                                    if (a.wref) go_eq(IC<fs.vec / 2>{}, IC<2 * fs.ty>{}, IC<1>{});
+                                    else go_eq(IC<fs.vec / 2>{}, IC<2 * fs.ty>{}, IC<0>{});
+                                } else {
+                                    if (a.wref) go_eq(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{});
+                                    else go_eq(IC<fs.vec>{}, IC<fs.ty>{}, IC<0>{});
+                                }
+                                if (done) return;
+                            }
                             // default: two stages of 8 rows.  Variant 12 = three stages of 6 rows (one component only: it
                             // decouples producers and consumers further but the smaller tile re-reads more; measured slower)
                             if (a.variant == 0) {

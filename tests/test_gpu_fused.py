@@ -34,7 +34,10 @@ def run_three(wl, inp, steps, oracle_wl=None):
     # k_fused_ws: D3Q19 and rows that are whole 16-byte vectors of the storage dtype; else the lock-step kernel
     sbytes = {"f16": 2, "f32": 4, "f64": 8}[wl.get("store_dtype", wl.get("compute_dtype", "f64"))]
     ws = wl["lattice"] == "D3Q19" and wl["nx"] % (16 // sbytes) == 0 and os.environ.get("LBM_TUNE_FUSED_VARIANT") != "-1"
-    want = "one_pass_ws" if ws else "one_pass_lockstep"
+    # ... and the row-pipeline kernel k_fused_eq where the collision result is an equilibrium (one component, BGK, tau = 1)
+    eq = ws and wl["n_components"] == 1 and wl.get("collision", "BGK") == "BGK" and list(wl.get("tau", [1.0])) == [1.0] \
+        and not os.environ.get("LBM_TUNE_NO_EQ")
+    want = "one_pass_eq" if eq else "one_pass_ws" if ws else "one_pass_lockstep"
     assert g1.hot_path == want, g1.hot_path        # and the intended kernel, not a silent fallback
     g2.step(steps)
     return ([o.get_populations(k) for k in range(o.nc)], [g1.get_populations(k) for k in range(o.nc)],

@@ -450,7 +450,7 @@ def test_body_force_periodic_d3q19(dtype, path):
     wl.update(nx=24, ny=10, nz=9, body_accel=(1e-4, -2e-4, 3e-4), path=path)
     inp = small_inputs(wl, 19, 0.05, 0.3)
     o, g, fo, fg = run_pair(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
-    assert g.hot_path == ("one_pass_ws" if path == "one_pass" else "two_pass")
+    assert g.hot_path == ("one_pass_eq" if path == "one_pass" else "two_pass")
     if dtype == "f64":
         assert_parity(fo, fg, fluid_mask(inp, o.N), TOL64, relative=False)
         assert np.abs(o.get_macroscopic()[1] - g.get_macroscopic()[1]).max() <= 1e-10
