@@ -43,7 +43,7 @@ struct lbm {
     int fvariant;        // tuning variant of K2F (0 = default)
     int fmchunk;         // planes marched per CTA
     bool use_fused;      // decided in prepare()
-    bool eq_narrow;      // k_fused_eq tile: 32 x VEC/2 cells by 16 rows instead of 32 x VEC by 8
+    bool eq_half;        // k_fused_eq with half-width tiles and two CTAs per SM
     bool feq;            // one component, BGK, tau = 1: the collision result is f_eq(rho, u' + du) (k_fused_eq applies)
     int last_path;       // lbm_hot_path: what the last lbm_step ran
     // launch-bound (small) domains: GRAPH_STEPS time steps captured once into a CUDA graph and replayed
@@ -561,7 +561,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.variant = h->fvariant;
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;
     a.pfd = 0;
-    a.eq = h->feq ? (h->eq_narrow ? 2 : 1) : 0;
+    a.eq = h->feq ? (h->eq_half ? 2 : 1) : 0;
     a.pdl = h->pdl ? 1 : 0;
     a.used_kernel = op == OP_FUSED ? &h->last_path : nullptr;
     if (const char* e = std::getenv("LBM_TUNE_FUSED_PFD")) a.pfd = std::atoi(e);
@@ -632,7 +632,7 @@ FusedShape fused_shape_of(const lbm_config_t& c, int variant) {
 void plan_fused(lbm* h) {
     h->use_fused = false;
     const lbm_config_t& c = h->cfg;
-    h->feq = c.n_components == 1 && c.collision == LBM_BGK && c.tau[0] == 1.0 && !std::getenv("LBM_TUNE_NO_EQ");
+    h->feq = false;
     if (c.flags & (LBM_FLAG_TWO_PASS | LBM_FLAG_NO_COLLIDE)) return;
     if (c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0)))
         return;   // Zhang-Chen weight / surface-tension source: two-pass path
@@ -640,21 +640,36 @@ void plan_fused(lbm* h) {
     if ((unsigned long long)c.n_components * h->q * (unsigned long long)h->plane >= (1ULL << 32)) return;   // 32-bit element offsets
     if (h->d == 3 && c.nx % (16 / (int)h->sbytes) != 0 && h->fvariant == 0) h->fvariant = -1;   // k_fused_ws copies 16-byte pads
     const int nm = h->d == 3 ? c.nz : c.ny;
-    const bool eq_tile = h->feq && h->d == 3 && h->fvariant == 0;
-    const int tx = h->fshape.wx * 32 * h->fshape.vec / (eq_tile && h->eq_narrow ? 2 : 1);
-    const int ty = h->fshape.ty * (eq_tile && h->eq_narrow ? 2 : 1);
+    // k_fused_eq: one component, BGK, tau = 1
+    h->feq = h->d == 3 && h->fvariant == 0 && c.n_components == 1 && c.collision == LBM_BGK && c.tau[0] == 1.0 &&
+             !std::getenv("LBM_TUNE_NO_EQ");
+    // half-width tiles, two CTAs per SM: where a full-width last tile would leave more than a tenth of the row's lanes idle
+    // and half-width tiles fewer, or where full-width tiles cannot give every SM a column (measured: 416^3 2.67 -> 2.59 ms,
+    // 128^3 0.0756 -> 0.0733; 512^3 3.9 -> 4.85: full width there)
+    {
+        const int txf = h->fshape.wx * 32 * h->fshape.vec, txh = txf / 2;
+        const double uf = (double)c.nx / (((c.nx + txf - 1) / txf) * (double)txf), uh = (double)c.nx / (((c.nx + txh - 1) / txh) * (double)txh);
+        const long long cols = (long long)((c.nx + txf - 1) / txf) * ((c.ny + h->fshape.ty - 1) / h->fshape.ty);
+        int nsm0 = 148;
+        cudaDeviceGetAttribute(&nsm0, cudaDevAttrMultiProcessorCount, 0);
+        if (!std::getenv("LBM_TUNE_EQ_HALF")) h->eq_half = h->fshape.vec >= 2 && ((uf < 0.9 && uh > uf + 0.05) || cols < nsm0 / 4);
+    }
+    const bool half = h->feq && h->eq_half;
+    const int tx = h->fshape.wx * 32 * h->fshape.vec / (half ? 2 : 1);
+    const int ty = h->fshape.ty;
     const long long tiles = (long long)((c.nx + tx - 1) / tx) * (h->d == 3 ? (c.ny + ty - 1) / ty : 1);
     // Chunks per column of tiles: every CTA pulls two extra planes and pays a few planes' worth of pipeline fill, and
     // CTAs run in waves of one per SM, so minimise  waves * (planes per chunk + 5)  (measured on 128^3 .. 512^3: the
     // model picks 16, 128 and 128 planes, the best of the sweeps in DESIGN.md 6)
     int nsm = 148;
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
+    const long long slots = (long long)nsm * (half ? 2 : 1);   // CTAs resident at a time
     long long best_cost = -1;
     int mchunk = nm;
     for (int nch = 1; nch <= std::max(1, nm / 8); ++nch) {
         const int mc = (nm + nch - 1) / nch;
         const long long ctas = tiles * ((nm + mc - 1) / mc);
-        const long long cost = ((ctas + nsm - 1) / nsm) * (mc + 5);
+        const long long cost = ((ctas + slots - 1) / slots) * (mc + 5);
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; mchunk = mc; }
     }
     if (const char* e = std::getenv("LBM_TUNE_FUSED_MCHUNK")) mchunk = std::max(1, std::min(nm, std::atoi(e)));
@@ -905,8 +920,8 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->fmchunk = 1;
     h->use_fused = false;
     h->feq = false;
-    h->eq_narrow = false;
-    if (const char* e = std::getenv("LBM_TUNE_EQ_NARROW")) h->eq_narrow = std::atoi(e) != 0;
+    h->eq_half = false;
+    if (const char* e = std::getenv("LBM_TUNE_EQ_HALF")) h->eq_half = std::atoi(e) != 0;
     h->last_path = LBM_PATH_NONE;
     h->gexec = nullptr;
     h->gcur = 0;

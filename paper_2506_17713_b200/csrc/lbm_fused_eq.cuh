@@ -21,17 +21,21 @@
 // Every row is its own two-slot pipeline; the warps meet only at the psi ring (one "plane complete" mbarrier per ring
 // slot, one "slot free" mbarrier for the halo / ring warps that run ahead).  The copies of plane pl+2 are in flight while
 // plane pl-1 is collided and plane pl+1 waits in the other slot.
-// Order inside a consumer iteration: the shared-memory loads of the NEXT plane are issued before the 19 global stores of
-// the collided plane, and what follows the stores is arithmetic only (moments, copy issue, psi): the stores drain
-// from the load/store queue while the warp computes instead of blocking the next plane's loads behind them (measured:
-// a quarter of the consumers' time was spent waiting for queued stores to release their registers).
+// CPS = 1: tiles of 32 x VEC cells by TY rows, one CTA per SM; CPS = 2: half-width tiles (VEC / 2 cells per lane), two CTAs
+// per SM -- chosen for rows that leave much of a full-width tile idle (416 = 3.25 x 128) and for domains with few tiles.
+// Measured on C5-512 and kept out: bulk copies issued by dedicated copy warps (same time: the consumers are
+// not issue-bound), one 4-D tensor-map box per direction instead of 190 row copies with either a TMA-stored staging
+// area (room for one landing slot only: 4.8 ms) or two landing slots (5.1 ms), the stores of a plane issued after the
+// shared-memory loads of the next (4.3 ms), stores per cell pair (half sectors: 5.1 ms).  What is left, from the stall
+// samples: the eight rows collide and store in the same phase, the 78 KB burst drains at ~40 B/cycle while the arithmetic
+// pipes idle (copies alone 1.9 ms, + arithmetic 2.9 ms, + stores 3.9 ms).
 // Arithmetic (order of every sum) is that of K1 / K2 in lbm_hot.cuh: results are bit-identical to the two-pass path.
 #pragma once
 #include "lbm_fused_ws.cuh"
 
 namespace lbmk {
 
-template <class L, class CT, class ST, int VEC, int TY>
+template <class L, class CT, class ST, int VEC, int TY, int CPS>
 struct EqTile {
     static_assert(L::D == 3, "the kernel marches along z");
     static constexpr int Q = L::Q;
@@ -55,18 +59,18 @@ struct EqTile {
     static constexpr int NBAR = NSTG * ROWS + 2 * NS;
     static constexpr size_t SMEM = sizeof(ST) * (NSTG * STAGE_ELEMS + 2 * NSTG * (size_t)RB) + sizeof(CT) * PSI_ELEMS + 8 * NBAR;
     // register split (setmaxnreg): the pool is THREADS x (registers at launch)
-    static constexpr int REG_LAUNCH = (65536 / THREADS) / 8 * 8;
-    static constexpr int REG_PROD = 56;
+    static constexpr int REG_LAUNCH = (65536 / CPS / THREADS) / 8 * 8;
+    static constexpr int REG_PROD = CPS == 1 ? 56 : 40;
     static constexpr int REG_CONS_ = ((REG_LAUNCH * THREADS - REG_PROD * NPW * 32) / (NCW * 32)) / 8 * 8;
     static constexpr int REG_CONS = REG_CONS_ > 232 ? 232 : REG_CONS_;
-    static_assert(SMEM <= 227 * 1024, "tile does not fit shared memory");
+    static_assert(SMEM <= (CPS == 1 ? 227 : 113) * 1024, "tile does not fit shared memory");
     static_assert(ROWS <= 32, "ring warps map one lane to one row");
 };
 
-template <class L, class CT, class ST, int VEC, int TY, bool WREF>
-__global__ void __launch_bounds__((EqTile<L, CT, ST, VEC, TY>::THREADS), 1)
+template <class L, class CT, class ST, int VEC, int TY, int CPS, bool WREF>
+__global__ void __launch_bounds__((EqTile<L, CT, ST, VEC, TY, CPS>::THREADS), CPS)
 k_fused_eq(const __grid_constant__ KParams<CT> p, int mchunk) {
-    using T = EqTile<L, CT, ST, VEC, TY>;
+    using T = EqTile<L, CT, ST, VEC, TY, CPS>;
     constexpr int Q = L::Q, NSTG = T::NSTG, NS = T::NS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     ST* stage = reinterpret_cast<ST*>(smem_raw);                          // [NSTG][TY][RB]
@@ -76,11 +80,7 @@ k_fused_eq(const __grid_constant__ KParams<CT> p, int mchunk) {
     uint64_t* bar_psi = bar_land + NSTG * T::ROWS;                         // [NS] psi of a plane complete
     uint64_t* bar_free = bar_psi + NS;                                     // [NS] ring slot read for the last time
 
-#ifndef LBM_EQ_NOSHFL
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // uniform, and known to be so
-#else
-    const int warp = threadIdx.x >> 5;
-#endif
     const int lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTG * T::ROWS; ++s) mbar_init(bar_land + s, 1);
@@ -154,9 +154,13 @@ k_fused_eq(const __grid_constant__ KParams<CT> p, int mchunk) {
         const bool used = cw < nint;
         const bool act = used && xl < txw;
         const unsigned cell0 = (unsigned)wrap_y(yb + cw) * sy + (unsigned)(tx0 + xl);
-        const RowPipe rp = make_pipe(r);
         auto slot_of = [&](int it) { return stage + (size_t)(it & 1) * T::STAGE_ELEMS + (size_t)cw * T::RB; };
-        // pulled populations of plane it: shared memory -> registers (issued early, consumed by moments_of)
+        const RowPipe rp = make_pipe(r);
+        if (used) {
+            issue(rp, r, 0, slot_of(0));
+            issue(rp, r, 1, slot_of(1));
+        }
+        // pulled populations of plane it: shared memory -> registers
         auto load_plane = [&](int it, CT (&A)[Q][VEC]) {
             const ST* rows = slot_of(it) + xl;
             static_for<0, Q>([&](auto I) {
@@ -178,10 +182,6 @@ k_fused_eq(const __grid_constant__ KParams<CT> p, int mchunk) {
             }
         };
         CT prho[VEC], pj[3][VEC];                          // the pending plane it-1: its moments
-        if (used) {
-            issue(rp, r, 0, slot_of(0));
-            issue(rp, r, 1, slot_of(1));
-        }
         for (int it = 0; it < nit; ++it) {
             CT rho[VEC], j[3][VEC];
             if (used) mbar_wait(bar_land + (it & 1) * T::ROWS + r, (it >> 1) & 1);
@@ -236,14 +236,8 @@ k_fused_eq(const __grid_constant__ KParams<CT> p, int mchunk) {
                             else A[I][v] = fc[I];
                         });
                     }
-#ifndef LBM_EQ_NOSTORE
                     ST* po = at_u32(static_cast<ST*>(p.f_out), (unsigned)wrap_m(m0 - 2 + it) * sz + cell0);
                     static_for<0, Q>([&](auto I) { st_vec_global<CT, ST, VEC>(po + (size_t)I * plane, A[I]); });
-#else
-                    CT acc = CT(0);
-                    static_for<0, Q>([&](auto I) { for (int v = 0; v < VEC; ++v) acc += A[I][v]; });
-                    if (acc == CT(123.456)) static_cast<ST*>(p.f_out)[cell0] = Cvt<CT, ST>::down(acc);
-#endif
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_free + (it - 2) % NS);   // plane it-2 of the ring has been read for the last time

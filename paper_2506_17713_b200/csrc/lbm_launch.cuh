@@ -31,7 +31,6 @@ struct LaunchArgs {
                          //           -1 = lock-step kernel everywhere; 1.. = tuning experiments (LBM_FUSED_TUNING)
     int pfd;             // OP_FUSED (warp-specialised): L2 prefetch distance in planes
     int eq;              // OP_FUSED: one component, BGK, tau = 1 (f* is an equilibrium): the row-pipeline kernel k_fused_eq applies
-                         //           1 = wide tile (32 x VEC cells by 8 rows), 2 = narrow tile (32 x VEC/2 cells by 16 rows)
     int* used_kernel;    // OP_FUSED, out: the lbm_path value of the kernel that ran
     int wref;            // OP_FUSED: rho_ref != 0 (populations stored shifted by w_i rho_ref)
     int pdl;             // OP_MOMENTS / OP_VIRTUAL / OP_STEP (dense mapping): programmatic dependent launch (pdl_begin)
@@ -257,10 +256,10 @@ cudaError_t launch(const LaunchArgs& a) {
                         }
                     };
                     // row-pipeline kernel (lbm_fused_eq.cuh): same tile, same opt-ins
-                    auto go_eq = [&](auto VEC, auto TY, auto WREF) {
+                    auto go_eq = [&](auto VEC, auto TY, auto CPS, auto WREF) {
                         if constexpr (L::D == 3 && NC == 1 && C_ == 0) {
-                            using T = EqTile<L, CT, ST, VEC, TY>;
-                            auto kern = k_fused_eq<L, CT, ST, VEC, TY, (WREF != 0)>;
+                            using T = EqTile<L, CT, ST, VEC, TY, CPS>;
+                            auto kern = k_fused_eq<L, CT, ST, VEC, TY, CPS, (WREF != 0)>;
                             static int ready[16] = {0};   // per device: 0 unknown, 1 usable, -1 not usable
                             int dev = 0;
                             cudaGetDevice(&dev);
@@ -287,12 +286,12 @@ cudaError_t launch(const LaunchArgs& a) {
                     if constexpr (fs.vec > 0) {
                         if constexpr (L::D == 3) {
                             if (a.variant == 0 && a.eq) {
-                                if (a.eq == 2) {
-                                    if (a.wref) go_eq(IC<fs.vec / 2>{}, IC<2 * fs.ty>{}, IC<1>{});
-                                    else go_eq(IC<fs.vec / 2>{}, IC<2 * fs.ty>{}, IC<0>{});
+                                if (a.eq == 2) {       // half-width tiles, two CTAs per SM
+                                    if (a.wref) go_eq(IC<fs.vec / 2>{}, IC<fs.ty>{}, IC<2>{}, IC<1>{});
+                                    else go_eq(IC<fs.vec / 2>{}, IC<fs.ty>{}, IC<2>{}, IC<0>{});
                                 } else {
-                                    if (a.wref) go_eq(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{});
-                                    else go_eq(IC<fs.vec>{}, IC<fs.ty>{}, IC<0>{});
+                                    if (a.wref) go_eq(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{}, IC<1>{});
+                                    else go_eq(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{}, IC<0>{});
                                 }
                                 if (done) return;
                             }
