@@ -229,6 +229,13 @@ KParams<CT> make_params(const lbm* h, int in_buf, int out_buf) {
                 for (int q2 = 0; q2 < 10; ++q2) p.mrt_ce[k][r][q2] = (CT)ce[r][q2];
             for (int r = 0; r < 9; ++r)
                 for (int q2 = 0; q2 < 9; ++q2) p.mrt_co[k][r][q2] = (CT)co[r][q2];
+            if (c.lattice == LBM_D3Q19)
+                for (int r = 0; r < 19; ++r) {
+                    const double n2 = (double)mrt_norm2<D3Q19>(r);
+                    p.mrt_c1[k][r] = (CT)((1.0 - c.mrt_rates[k][r]) / n2);
+                    p.mrt_c2[k][r] = (CT)(c.mrt_rates[k][r] / n2);
+                    p.mrt_c3[r] = (CT)(1.0 / n2);
+                }
         }
         const lbm_eos_t& e = c.eos[k];
         p.psi_kind[k] = e.psi_kind;

@@ -149,6 +149,7 @@ struct KParams {
     CT G[2][2];
     CT mrt_ce[2][10][10];  // MRT: M^-1 S M restricted to the even subspace (rest + direction pairs), lbm_hot.cuh
     CT mrt_co[2][9][9];    //      ... and to the odd subspace (pair differences)
+    CT mrt_c1[2][19], mrt_c2[2][19], mrt_c3[19];   // D3Q19 MRT in moment space: (1 - s_r)/|M_r|^2, s_r/|M_r|^2, 1/|M_r|^2
     CT c_feq_a[2], c_feq_b[2], c_keep[2];  // f* = c_keep f + c_feq_a feq(u_a) + c_feq_b feq(u + du)  (BGK; lbm_hot.cuh)
     CT wref[19];       // w_i * rho_ref
     int psi_kind[2];

@@ -276,13 +276,119 @@ __device__ __forceinline__ void add_feq(CT coef, CT rho, const CT (&u)[3], CT (&
     });
 }
 
+// D3Q19 equilibrium moments m_eq = M f_eq(rho, u) in closed form (R9: d'Humieres basis, f_eq of R1; the same expressions
+// are held to the oracle's matrix product in tests/test_oracle_basics.py::test_d3q19_equilibrium_moments_closed_form, the
+// kernel to the oracle's dense M^-1 S M by the fp64 parity tests): row order of mrt_entry2<D3Q19>.
+template <class CT>
+__device__ __forceinline__ void meq_d3q19(CT rho, const CT (&u)[3], CT (&m)[19]) {
+    const CT jx = rho * u[0], jy = rho * u[1], jz = rho * u[2];
+    const CT xx = jx * u[0], yy = jy * u[1], zz = jz * u[2];
+    const CT ruu = xx + yy + zz;
+    m[0] = rho;
+    m[1] = CT(19) * ruu - CT(11) * rho;
+    m[2] = CT(3) * rho - CT(5.5) * ruu;
+    m[3] = jx; m[4] = CT(-2.0 / 3.0) * jx;
+    m[5] = jy; m[6] = CT(-2.0 / 3.0) * jy;
+    m[7] = jz; m[8] = CT(-2.0 / 3.0) * jz;
+    m[9] = CT(2) * xx - yy - zz;
+    m[10] = CT(-0.5) * m[9];
+    m[11] = yy - zz;
+    m[12] = CT(-0.5) * m[11];
+    m[13] = jx * u[1];
+    m[14] = jy * u[2];
+    m[15] = jx * u[2];
+    m[16] = m[17] = m[18] = CT(0);
+}
+
+// S6, MRT on D3Q19 in moment space (Eq. 3 second line):  f* = M^-1 [ m - S (m - m_eq(u_a)) (+ m_eq(u_b) - m_eq(u') for
+// EDM, Eq. 5) ].  The rows of M are even or odd polynomials of c, so the transform splits into the pair sums (10 even
+// moments) and the pair differences (9 odd moments); its integer entries (0, +-1, +-2, +-4, 8, -11, 12, -30) are factored by
+// hand: ~50 additions forward, ~90 multiply-adds back, instead of the 181 multiply-adds of the dense even / odd blocks plus
+// a second 19-term f_eq.  c1 = (1 - s_r) / |M_r|^2, c2 = s_r / |M_r|^2, c3 = 1 / |M_r|^2 come from the host.
+template <class CT>
+__device__ __forceinline__ void collide_mrt_d3q19(const KParams<CT>& p, int k, CT rho, const CT (&u)[3], const CT (&ua)[3],
+                                                  const CT (&ub)[3], bool edm, CT (&f)[19]) {
+    (void)u;   // EDM: u_a = u'
+    // pair sums / differences: x, y, z, xy+, xy-, xz+, xz-, yz+, yz-  (directions 2P+1, 2P+2)
+    const CT sx = f[1] + f[2], sy = f[3] + f[4], sz = f[5] + f[6];
+    const CT sa = f[7] + f[8], sb = f[9] + f[10], sc = f[11] + f[12], sd = f[13] + f[14], sg = f[15] + f[16], sh = f[17] + f[18];
+    const CT dx = f[1] - f[2], dy = f[3] - f[4], dz = f[5] - f[6];
+    const CT da = f[7] - f[8], db = f[9] - f[10], dc = f[11] - f[12], dd = f[13] - f[14], dg = f[15] - f[16], dh = f[17] - f[18];
+    CT m[19];
+    {   // even moments
+        const CT A = sx + sy + sz, Sxy = sa + sb, Sxz = sc + sd, Syz = sg + sh, D = Sxy + Sxz + Syz;
+        const CT t9 = Sxy + Sxz - CT(2) * Syz, t11 = Sxy - Sxz;
+        const CT ax = CT(2) * sx - sy - sz, aw = sy - sz;
+        m[0] = f[0] + A + D;
+        m[1] = CT(8) * D - CT(11) * A - CT(30) * f[0];
+        m[2] = D - CT(4) * A + CT(12) * f[0];
+        m[9] = ax + t9;
+        m[10] = t9 - CT(2) * ax;
+        m[11] = aw + t11;
+        m[12] = t11 - CT(2) * aw;
+        m[13] = sa - sb;
+        m[14] = sg - sh;
+        m[15] = sc - sd;
+    }
+    {   // odd moments
+        const CT ox = da + db + dc + dd, oy = da - db + dg + dh, oz = dc - dd + dg - dh;
+        m[3] = dx + ox; m[4] = ox - CT(4) * dx;
+        m[5] = dy + oy; m[6] = oy - CT(4) * dy;
+        m[7] = dz + oz; m[8] = oz - CT(4) * dz;
+        m[16] = da + db - dc - dd;
+        m[17] = db - da + dg + dh;
+        m[18] = dc - dd - dg + dh;
+    }
+    // relaxation towards m_eq(u_a), EDM source m_eq(u_b) - m_eq(u'); the result is already divided by |M_r|^2
+    CT me[19];
+    meq_d3q19<CT>(rho, ua, me);
+    static_for<0, 19>([&](auto R) { m[R] = p.mrt_c1[k][R] * m[R] + p.mrt_c2[k][R] * me[R]; });
+    if (edm) {
+        CT mb[19];
+        meq_d3q19<CT>(rho, ub, mb);
+        static_for<1, 16>([&](auto R) { m[R] += p.mrt_c3[R] * (mb[R] - me[R]); });
+    }
+    // back: f = M^T m
+    {
+        const CT base_a = m[0] - CT(11) * m[1] - CT(4) * m[2];      // axis directions
+        const CT base_d = m[0] + CT(8) * m[1] + m[2];               // diagonals
+        const CT q9 = m[9] + m[10], q11 = m[11] + m[12];
+        const CT ex_ = base_a + CT(2) * m[9] - CT(4) * m[10];
+        const CT ey_ = base_a - m[9] + CT(2) * m[10] + m[11] - CT(2) * m[12];
+        const CT ez_ = base_a - m[9] + CT(2) * m[10] - m[11] + CT(2) * m[12];
+        const CT exy = base_d + q9 + q11, exz = base_d + q9 - q11, eyz = base_d - CT(2) * q9;
+        const CT ox_ = m[3] - CT(4) * m[4], oy_ = m[5] - CT(4) * m[6], oz_ = m[7] - CT(4) * m[8];
+        const CT jqx = m[3] + m[4], jqy = m[5] + m[6], jqz = m[7] + m[8];
+        f[0] = m[0] - CT(30) * m[1] + CT(12) * m[2];
+        f[1] = ex_ + ox_; f[2] = ex_ - ox_;
+        f[3] = ey_ + oy_; f[4] = ey_ - oy_;
+        f[5] = ez_ + oz_; f[6] = ez_ - oz_;
+        {   // (1,1,0) / (1,-1,0)
+            const CT ea = exy + m[13], eb = exy - m[13];
+            const CT oa = jqx + jqy + m[16] - m[17], ob = jqx - jqy + m[16] + m[17];
+            f[7] = ea + oa; f[8] = ea - oa; f[9] = eb + ob; f[10] = eb - ob;
+        }
+        {   // (1,0,1) / (1,0,-1)
+            const CT ea = exz + m[15], eb = exz - m[15];
+            const CT oa = jqx + jqz - m[16] + m[18], ob = jqx - jqz - m[16] - m[18];
+            f[11] = ea + oa; f[12] = ea - oa; f[13] = eb + ob; f[14] = eb - ob;
+        }
+        {   // (0,1,1) / (0,1,-1)
+            const CT ea = eyz + m[14], eb = eyz - m[14];
+            const CT oa = jqy + jqz + m[17] - m[18], ob = jqy - jqz + m[17] + m[18];
+            f[15] = ea + oa; f[16] = ea - oa; f[17] = eb + ob; f[18] = eb - ob;
+        }
+    }
+}
+
 // S6 for one cell and one component.  u: common velocity u' (R6); du = F/rho (Eq. 5).
 //   BGK : f* = c_keep f + c_feq_a f_eq(u_a) + c_feq_b f_eq(u' + du)
 //         EDM   (Eq. 3 + Eq. 5): u_a = u', c_keep = 1 - 1/tau, c_feq_a = 1/tau - 1, c_feq_b = 1
 //         SHIFT (R7)           : u_a = u' + tau du, c_keep = 1 - 1/tau, c_feq_a = 1/tau, c_feq_b = 0
-//   MRT : f* = f - M^-1 S M (f - f_eq(u_a)) [+ f_eq(u' + du) - f_eq(u') for EDM], with M^-1 S M applied as its
-//         even block (on f_0 and the pair sums) and odd block (on the pair differences): rows of M are even or
-//         odd polynomials of c (R9), so M^-1 S M = C_even + C_odd with no cross terms.
+//   MRT : f* = f - M^-1 S M (f - f_eq(u_a)) [+ f_eq(u' + du) - f_eq(u') for EDM].  D3Q19: in moment space with the
+//         hand-factored transform (collide_mrt_d3q19).  D2Q9: M^-1 S M applied as its even block (on f_0 and the pair
+//         sums) and odd block (on the pair differences): rows of M are even or odd polynomials of c (R9), so
+//         M^-1 S M = C_even + C_odd with no cross terms.
 template <class L, int COLL, class CT>
 __device__ __forceinline__ void collide(const KParams<CT>& p, int k, CT rho, const CT (&u)[3], const CT (&du)[3],
                                         CT (&f)[L::Q]) {
@@ -305,6 +411,8 @@ __device__ __forceinline__ void collide(const KParams<CT>& p, int k, CT rho, con
             if (ca != CT(0)) add_feq<L, CT>(ca, rho, ua, f);
             if (cb != CT(0)) add_feq<L, CT>(cb, rho, ub, f);
         }
+    } else if constexpr (L::D == 3) {
+        collide_mrt_d3q19<CT>(p, k, rho, u, ua, ub, !shift, f);
     } else {
         CT e[L::Q];
         static_for<0, L::Q>([&](auto I) { e[I] = CT(0); });

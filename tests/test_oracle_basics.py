@@ -90,6 +90,24 @@ def test_mrt_basis(name):
     assert np.allclose(M[srows] @ w, 0, atol=1e-15)
 
 
+def test_d3q19_equilibrium_moments_closed_form():
+    """m_eq = M f_eq (Eq. 3 taken literally, R9) has the textbook closed form of d'Humieres et al. (2002) with the
+    second-order f_eq: e = -11 rho + 19 rho u^2, eps = 3 rho - 11/2 rho u^2, q = -2/3 j, 3 p_xx = rho (2 ux^2 - uy^2 - uz^2),
+    3 pi_xx = -1/2 * 3 p_xx, p_ww = rho (uy^2 - uz^2), pi_ww = -1/2 p_ww, p_xy = rho ux uy, ..., m = 0.  Pins the row order
+    and the signs of the oracle's D3Q19 basis (and the expressions the CUDA path evaluates instead of the product)."""
+    M, _ = o.mrt_matrices("D3Q19")
+    rng = np.random.default_rng(12)
+    for _ in range(10):
+        rho = rng.uniform(0.05, 8.0)
+        ux, uy, uz = rng.uniform(-0.12, 0.12, 3)
+        uu = ux * ux + uy * uy + uz * uz
+        pxx, pww = rho * (2 * ux * ux - uy * uy - uz * uz), rho * (uy * uy - uz * uz)
+        expect = np.array([rho, rho * (19 * uu - 11), rho * (3 - 5.5 * uu), rho * ux, -2 / 3 * rho * ux, rho * uy, -2 / 3 * rho * uy,
+                           rho * uz, -2 / 3 * rho * uz, pxx, -0.5 * pxx, pww, -0.5 * pww, rho * ux * uy, rho * uy * uz, rho * ux * uz,
+                           0, 0, 0])
+        assert np.abs(M @ o.feq("D3Q19", rho, [ux, uy, uz]) - expect).max() < 1e-14 * rho * 30
+
+
 # ------------------------------------------------------------------ fp16 storage rounding (R16)
 def test_round_to_half_matches_numpy_float16():
     rng = np.random.default_rng(1)
