@@ -779,7 +779,8 @@ int prepare(lbm* h) {
     // Compact mode (lbm_compact.cuh): a quarter or less of the cells fluid, plain Shan-Chen force
     const lbm_config_t& c = h->cfg;
     const bool ext_force = c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0));
-    h->compact_on = h->use_list && !ext_force && h->nfluid <= h->N / 4 && (long long)h->nfluid + h->nbsolid <= h->N;
+    h->compact_on = h->use_list && !ext_force && h->nfluid <= h->N / 4 && (long long)h->nfluid + h->nbsolid <= h->N &&
+                    (long long)h->nfluid + h->nbsolid < (1LL << 28);   // 28-bit extended indices in the neighbour table
     if (const char* e = std::getenv("LBM_TUNE_COMPACT")) h->compact_on = h->compact_on && std::atoi(e) != 0;
     if (h->compact_on && (unsigned long long)h->q * (((unsigned long long)h->nfluid + 63) / 64 * 64) >= (1ULL << 32))
         h->compact_on = false;   // 32-bit element offsets within a component
@@ -801,28 +802,17 @@ int prepare(lbm* h) {
 }
 
 // Bring the current population buffer into the fluid-compact (lbm_step on porous domains) or the dense layout (every
-// other entry point): a copy through the other buffer.
+// other entry point): a gather / scatter through the other buffer.
 int set_layout(lbm* h, bool compact) {
     if (!h->initialized || h->is_compact == compact) return LBM_OK;
-    const char* src = h->ws + h->cv.f[h->cur];
-    char* dst = h->ws + h->cv.f[h->cur ^ 1];
-    const int* flist = reinterpret_cast<const int*>(h->ws + h->cv.flist);
-    const int np = h->cfg.n_components * h->q;
-    const unsigned grid = (unsigned)((h->nfluid + 255) / 256);
     int rc;
     if (!compact) {
         h->is_compact = false;   // the fill below is a dense kernel
         if ((rc = do_launch(h, OP_FILL_SOLID))) return rc;
         CU(cudaMemsetAsync(h->ws + h->cv.psi, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));
     }
-    if (h->sbytes == 2)
-        k_pack<uint16_t><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint16_t*>(src), reinterpret_cast<uint16_t*>(dst), flist, h->nfluid, h->plane, h->nbr_stride, np, compact ? 0 : 1);
-    else if (h->sbytes == 4)
-        k_pack<uint32_t><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const uint32_t*>(src), reinterpret_cast<uint32_t*>(dst), flist, h->nfluid, h->plane, h->nbr_stride, np, compact ? 0 : 1);
-    else
-        k_pack<unsigned long long><<<grid, 256, 0, h->stream>>>(reinterpret_cast<const unsigned long long*>(src), reinterpret_cast<unsigned long long*>(dst), flist, h->nfluid, h->plane, h->nbr_stride, np, compact ? 0 : 1);
-    CU(cudaGetLastError());
-    h->launches++;
+    // dense planes hold post-collision values at the writing cell, compact planes post-stream values (lbm_compact.cuh)
+    if ((rc = do_launch(h, compact ? OP_PACK_C : OP_UNPACK_C))) return rc;
     h->cur ^= 1;
     h->is_compact = compact;
     return LBM_OK;

@@ -4,20 +4,26 @@
 // nobody reads.  While lbm_step runs on such a domain the populations therefore live in the order of the fluid-cell list:
 // slot n of a direction plane belongs to the n-th fluid cell (ascending cell index; the planes are cplane = nfluid rounded
 // up to 64 elements apart, so the whole state is one contiguous block), and psi lives in "extended" order
-// (slots [0, nfluid) = fluid cells, [nfluid, nfluid + nbsolid) = boundary solids in the order of their list).  One
-// neighbour table nbr[(i-1) * nbr_stride + n] (i = 1 .. Q-1) holds the extended index of the cell at x + e_i (wrap, or the
-// clamped cell of R10 with bit 31 set when the link crosses a non-periodic face).  It serves both stencils:
-//   pull of direction i   : source x - e_i = x + e_ibar -> nbr[ibar]; a fluid index (< nfluid, bit 31 clear) is read,
-//                           anything else is a flagged link (halfway bounce-back: own stored_ibar)
-//   psi of neighbour x+e_i: psi_ext[nbr[i] & 0x7fffffff]
+// (slots [0, nfluid) = fluid cells, [nfluid, nfluid + nbsolid) = boundary solids in the order of their list).
+// In this layout the planes hold the POST-STREAM populations f_i(x_n, t) ("push" streaming): K1 and K2 read nothing but
+// their own slot of every plane -- coalesced, no index in front of the loads -- and K2 scatters f*_i to the slot of the
+// cell at x + e_i, or, when that cell is not fluid (halfway bounce-back, faces), to its own slot of plane ibar.  One
+// neighbour table nbr[(i-1) * nbr_stride + n] (i = 1 .. Q-1) holds, in its low 28 bits, the extended index of the cell at
+// x + e_i (wrap, or the clamped cell of R10; when the link crosses a non-periodic face bit 31 is set and bits 28-30 name the
+// face, lowest axis first); K2 alone reads it, for the psi gather psi_ext[nbr[i] & NBR_IDX], as the scatter address and
+// for the velocity / pressure rules of face links (no cell coordinates, flags or fluid list in the hot loop).  Every slot of a plane is written exactly once per step
+// (by the one cell that streams or bounces into it), so the scatter is race-free and leaves no stale value.
 // The arithmetic is the dense kernels' (same device functions, same order), so the results are bit-identical to the
-// dense layout; every other entry point works on the dense layout (k_pack / k_unpack convert at the boundary).
+// dense layout; every other entry point works on the dense layout, whose planes hold post-collision values at the
+// writing cell (lbm_core.cuh): k_pack_c pulls them into compact order, k_unpack_c scatters them back.
 #pragma once
-#include "lbm_hot.cuh"
+#include "lbm_fused_ws.cuh"   // mbarrier / bulk-copy primitives
 
 namespace lbmk {
 
-constexpr uint32_t NBR_FACE = 0x80000000u;
+constexpr uint32_t NBR_FACE = 0x80000000u;   // the link crosses a non-periodic face ...
+constexpr int NBR_FACE_SHIFT = 28;          // ... this one (3 bits)
+constexpr uint32_t NBR_IDX = 0x0fffffffu;    // extended index of the neighbour
 
 // neighbour table from the dense -> extended index map (cmap: -1 for solids that touch no fluid cell)
 template <class L, class CT>
@@ -31,19 +37,19 @@ __global__ void __launch_bounds__(256) k_build_nbr(const __grid_constant__ KPara
     static_for<1, L::Q>([&](auto I) {
         constexpr int i = I;
         int pc[3] = {x + L::E[i][0], y + L::E[i][1], z + L::E[i][2]};
-        bool crossed = false;
+        int face = -1;   // lowest axis first, as crossed_face() and the oracle's pull_source
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             if (pc[a] < 0) {
                 if (p.periodic[a]) pc[a] += dims[a];
-                else { pc[a] = 0; crossed = true; }
+                else { pc[a] = 0; if (face < 0) face = 2 * a; }
             } else if (pc[a] >= dims[a]) {
                 if (p.periodic[a]) pc[a] -= dims[a];
-                else { pc[a] = dims[a] - 1; crossed = true; }
+                else { pc[a] = dims[a] - 1; if (face < 0) face = 2 * a + 1; }
             }
         }
         const uint32_t e = (uint32_t)__ldg(cmap + pc[0] + p.nx * (pc[1] + p.ny * pc[2]));
-        nbr[(long long)(i - 1) * p.nbr_stride + n] = (e & ~NBR_FACE) | (crossed ? NBR_FACE : 0u);
+        nbr[(long long)(i - 1) * p.nbr_stride + n] = (e & NBR_IDX) | (face >= 0 ? NBR_FACE | ((uint32_t)face << NBR_FACE_SHIFT) : 0u);
     });
 }
 
@@ -52,16 +58,50 @@ static __global__ void __launch_bounds__(256) k_cmap_scatter(int n, const int* _
     if (t < n) cmap[list[t]] = base + t;
 }
 
-// dense -> compact / compact -> dense copies of every population plane (T = raw storage element)
-template <class T>
-__global__ void __launch_bounds__(256) k_pack(const T* __restrict__ src, T* __restrict__ dst, const int* __restrict__ flist,
-                                             int nfluid, long long plane, long long cplane, int nplanes, int to_dense) {
+// dense (post-collision at the writing cell) -> compact (post-stream): the pull of lbm_core.cuh on raw storage values
+template <class L, int NC, class CT, class ST>
+__global__ void __launch_bounds__(256) k_pack_c(const __grid_constant__ KParams<CT> p) {
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= nfluid) return;
-    const int id = __ldg(flist + n);
-    const long long from = to_dense ? n : id, to = to_dense ? id : n;
-    const long long sp = to_dense ? cplane : plane, dp = to_dense ? plane : cplane;
-    for (int pl = 0; pl < nplanes; ++pl) dst[pl * dp + to] = src[pl * sp + from];
+    if (n >= p.nfluid) return;
+    const int id = __ldg(p.flist + n);
+    const uint32_t fl = __ldg(p.flags + id);
+    const Cell c = make_cell<L>(p, id);
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        const ST* in = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.plane + id;
+        ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.cplane + n;
+        static_for<0, L::Q>([&](auto I) {
+            constexpr int i = I;
+            constexpr int ib = opposite<L>(i);
+            if constexpr (i == 0) out[0] = in[0];
+            else out[(long long)i * p.cplane] = ((fl >> i) & 1u) ? in[(long long)ib * p.plane]
+                                                                   : in[(long long)i * p.plane + nbr_offset<-L::E[i][0], -L::E[i][1], -L::E[i][2]>(c)];
+        });
+    }
+}
+
+// compact (post-stream) -> dense (post-collision at the writing cell): the scatter of k_unstream; every fluid slot of the
+// dense planes is written exactly once, the solid ones by k_fill_solid
+template <class L, int NC, class CT, class ST>
+__global__ void __launch_bounds__(256) k_unpack_c(const __grid_constant__ KParams<CT> p) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= p.nfluid) return;
+    const int id = __ldg(p.flist + n);
+    const uint32_t fl = __ldg(p.flags + id);
+    const Cell c = make_cell<L>(p, id);
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        const ST* in = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.cplane + n;
+        ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.plane + id;
+        static_for<0, L::Q>([&](auto I) {
+            constexpr int i = I;
+            constexpr int ib = opposite<L>(i);
+            const ST v = in[(long long)i * p.cplane];
+            if constexpr (i == 0) out[0] = v;
+            else if ((fl >> i) & 1u) out[(long long)ib * p.plane] = v;
+            else out[(long long)i * p.plane + nbr_offset<-L::E[i][0], -L::E[i][1], -L::E[i][2]>(c)] = v;
+        });
+    }
 }
 
 // solid cells of the dense layout hold f_eq(1, 0) (include/lbm.h, lbm_init_fields)
@@ -87,38 +127,25 @@ __device__ __forceinline__ void load_nbr(const KParams<CT>& p, unsigned n, uint3
     static_for<1, L::Q>([&](auto I) { nb[I] = __ldg(p.nbr + (long long)(I - 1) * p.nbr_stride + n); });
 }
 
-// S7 read side in compact order: f[i] = stored_i(x - e_i), or stored_ibar(x) on a flagged link
+// the Q populations that have arrived at fluid cell n: its own slot of every plane
 template <class L, class CT, class ST>
-__device__ __forceinline__ void pull_compact(const KParams<CT>& p, unsigned n, const uint32_t (&nb)[L::Q], int k, CT (&f)[L::Q]) {
+__device__ __forceinline__ void load_compact(const KParams<CT>& p, unsigned n, int k, CT (&f)[L::Q]) {
     // 32-bit element offsets within a component (Q * cplane < 2^32 is a condition of the mode)
     const ST* base = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.cplane;
     const uint32_t cp = (uint32_t)p.cplane;
-    static_for<0, L::Q>([&](auto I) {
-        constexpr int i = I;
-        if constexpr (i == 0) {
-            f[0] = ld_one<CT, ST>(base + n) + p.wref[0];
-        } else {
-            constexpr int ib = opposite<L>(i);
-            const uint32_t s = nb[ib];
-            const bool ok = s < (uint32_t)p.nfluid;
-            const uint32_t off = ok ? (uint32_t)i * cp + s : (uint32_t)ib * cp + n;
-            f[i] = ld_one<CT, ST>(base + off) + p.wref[i];
-        }
-    });
+    static_for<0, L::Q>([&](auto I) { f[I] = ld_one<CT, ST>(base + ((uint32_t)I * cp + n)) + p.wref[I]; });
 }
 
-// ------------------------------------------------------------------ K1 in compact order
+// ------------------------------------------------------------------ K1 in compact order: a streaming read, no table
 template <class L, int NC, class CT, class ST>
 __global__ void __launch_bounds__(256, 4) k_moments_c(const __grid_constant__ KParams<CT> p) {
     const unsigned n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= (unsigned)p.nfluid) return;
-    uint32_t nb[L::Q];
-    load_nbr<L, CT>(p, n, nb);
     const int id = p.write_rho ? __ldg(p.flist + n) : 0;
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
         CT f[L::Q];
-        pull_compact<L, CT, ST>(p, n, nb, k, f);
+        load_compact<L, CT, ST>(p, n, k, f);
         const CT r = density<L, CT>(f);
         p.psi[(long long)k * p.N + n] = psi_of_rho(p, k, r);
         if (p.write_rho) p.rho[(long long)k * p.N + id] = r;   // dense: K1b averages it around the boundary solids
@@ -126,52 +153,73 @@ __global__ void __launch_bounds__(256, 4) k_moments_c(const __grid_constant__ KP
 }
 
 // ------------------------------------------------------------------ K2 in compact order
-// One cell per thread and gathers everywhere: the kernel lives on warps in flight.  With two components the 2 x Q
-// pulled populations are parked in shared memory ([component][direction][thread], conflict-free, private to the
-// thread: no barrier) between the moment sums and the collision, which keeps the kernel at 64 .. 100 registers
-// (five to eight CTAs per SM instead of four at 128 registers).
-#ifndef LBM_COMPACT_PARK
-#define LBM_COMPACT_PARK 1
-#endif
-// CTAs per SM (measured on config 4, 400^3: fp32 store 1.46 ms at 5 against 1.52 at 8; fp16 store 1.29 at 8, 1.41 at 5)
-#ifndef LBM_COMPACT_CTAS
-#define LBM_COMPACT_CTAS (sizeof(ST) == 2 ? 8 : 5)
-#endif
-template <class L, int NC, class CT, class ST, int COLL>
-__global__ void __launch_bounds__(128, ((NC == 2 && LBM_COMPACT_PARK) || sizeof(ST) == 2 ? LBM_COMPACT_CTAS : 1))
-k_step_c(const __grid_constant__ KParams<CT> p) {
-    constexpr bool PARK = NC == 2 && LBM_COMPACT_PARK;
-    __shared__ CT park[PARK ? NC * L::Q * 128 : 1];
-    const unsigned n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= (unsigned)p.nfluid) return;
-    uint32_t nb[L::Q];
-    load_nbr<L, CT>(p, n, nb);
+// A CTA owns CB consecutive fluid cells.  In compact order its Q populations per component and its Q-1 table rows are
+// NC*Q + Q-1 contiguous runs of CB elements: they are brought into shared memory by bulk asynchronous copies (TMA unit,
+// one request per run, all in flight at once, no registers), where the direct loads needed three dependent round
+// trips under the register cap (table + first component, second component, psi gathers) and 40 % of the instructions
+// were address arithmetic (profiles/r02_*).  What hangs on the table -- the psi gathers and the scatter addresses -- is
+// issued as soon as the copies have landed; several CTAs per SM hide that second round trip.
+template <class L, int NC, class ST>
+struct CompactTile {
+    static constexpr int CB = 128;                                  // cells per CTA = threads
+    static constexpr int NPOP = NC * L::Q;                          // population runs
+    static constexpr int NTAB = L::Q - 1;                           // table rows
+    static constexpr size_t POP_BYTES = (size_t)NPOP * CB * sizeof(ST);
+    static constexpr size_t TAB_BYTES = (size_t)NTAB * CB * 4;
+    static constexpr size_t SMEM = POP_BYTES + TAB_BYTES + 16;
+};
 
-    CT f[PARK ? 1 : NC][L::Q], rho[NC], j[NC][3];
-#pragma unroll
-    for (int k = 0; k < NC; ++k) {
-        CT(&fk)[L::Q] = f[PARK ? 0 : k];
-        pull_compact<L, CT, ST>(p, n, nb, k, fk);
-        if constexpr (COLL != 2) moments<L, CT>(fk, rho[k], j[k]);
-        if constexpr (PARK) static_for<0, L::Q>([&](auto I) { park[(k * L::Q + I) * 128 + threadIdx.x] = fk[I]; });
+template <class L, int NC, class CT, class ST, int COLL>
+__global__ void __launch_bounds__(128, (sizeof(ST) == 2 ? 8 : 6)) k_step_c(const __grid_constant__ KParams<CT> p) {
+    using T = CompactTile<L, NC, ST>;
+    constexpr int Q = L::Q, CB = T::CB;
+    extern __shared__ __align__(16) unsigned char smem_c[];
+    ST* pops = reinterpret_cast<ST*>(smem_c);                                   // [NC * Q][CB]
+    uint32_t* tab = reinterpret_cast<uint32_t*>(smem_c + T::POP_BYTES);         // [Q - 1][CB]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_c + T::POP_BYTES + T::TAB_BYTES);
+    const unsigned n0 = blockIdx.x * CB;
+    const unsigned t = threadIdx.x;
+    const unsigned n = n0 + t;
+    // the planes are padded to cplane (a multiple of 64 elements), so the last CTA may copy up to the padded end
+    const unsigned cnt = min((unsigned)CB, (unsigned)p.cplane - n0);
+    if (t == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    CT u[3] = {CT(0), CT(0), CT(0)}, du[NC][3];
+    __syncthreads();
+    if (t == 0) mbar_expect_tx(bar, cnt * (uint32_t)(T::NPOP * sizeof(ST) + T::NTAB * 4));
+    __syncthreads();
+    if (t < T::NPOP) {
+        const int k = t / Q, i = t - k * Q;
+        const ST* src = static_cast<const ST*>(p.f_in) + ((long long)k * Q * p.cplane + (long long)i * p.cplane + n0);
+        bulk_g2s(pops + t * CB, src, cnt * (uint32_t)sizeof(ST), bar);
+    } else if (t < T::NPOP + T::NTAB) {
+        const int i = t - T::NPOP;
+        bulk_g2s(tab + i * CB, p.nbr + ((long long)i * p.nbr_stride + n0), cnt * 4u, bar);
+    }
+    mbar_wait(bar, 0);
+    if (n >= (unsigned)p.nfluid) return;
+
+    uint32_t nb[Q];
+    nb[0] = n;
+    static_for<1, Q>([&](auto I) { nb[I] = tab[(I - 1) * CB + t]; });
+    // psi gathers first: the second (and last) round trip to memory
+    CT S[NC][3], pc[NC];
     if constexpr (COLL != 2) {
-        CT S[NC][3], pc[NC];
 #pragma unroll
         for (int kp = 0; kp < NC; ++kp) {
             const CT* ps = p.psi + (long long)kp * p.N;
-            auto rowfn = [&](auto DY, auto DZ, auto NX, CT (&t)[1], CT& left, CT& right) {
+            auto rowfn = [&](auto DY, auto DZ, auto NX, CT (&tv)[1], CT& left, CT& right) {
                 constexpr int dy = DY, dz = DZ;
-                if constexpr (dy == 0 && dz == 0) t[0] = __ldg(ps + n);
+                if constexpr (dy == 0 && dz == 0) tv[0] = __ldg(ps + n);
                 else if constexpr (row_has<L>(dy, dz, 0)) {
                     constexpr int i0 = dir_of<L>(0, dy, dz);   // constexpr locals: the lattice tables are host data
-                    t[0] = __ldg(ps + (nb[i0] & ~NBR_FACE));
+                    tv[0] = __ldg(ps + (nb[i0] & NBR_IDX));
                 }
                 if constexpr (NX != 0) {
                     constexpr int im = dir_of<L>(-1, dy, dz), ip = dir_of<L>(1, dy, dz);
-                    left = __ldg(ps + (nb[im] & ~NBR_FACE));
-                    right = __ldg(ps + (nb[ip] & ~NBR_FACE));
+                    left = __ldg(ps + (nb[im] & NBR_IDX));
+                    right = __ldg(ps + (nb[ip] & NBR_IDX));
                 }
             };
             CT S1[3][1], pc1[1];
@@ -179,26 +227,45 @@ k_step_c(const __grid_constant__ KParams<CT> p) {
             S[kp][0] = S1[0][0]; S[kp][1] = S1[1][0]; S[kp][2] = S1[2][0];
             pc[kp] = pc1[0];
         }
+    }
+    auto load_pops = [&](int k, CT (&fk)[Q]) {
+        static_for<0, Q>([&](auto I) { fk[I] = Cvt<CT, ST>::up(pops[(k * Q + I) * CB + t]) + p.wref[I]; });
+    };
+    CT rho[NC], j[NC][3];
+    CT u[3] = {CT(0), CT(0), CT(0)}, du[NC][3];
+    if constexpr (COLL != 2) {
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            CT fk[Q];
+            load_pops(k, fk);
+            moments<L, CT>(fk, rho[k], j[k]);
+        }
         force_and_velocity<NC, CT>(p, rho, j, S, pc, u, du);
     }
     uint32_t anyface = 0;
-    static_for<1, L::Q>([&](auto I) { anyface |= nb[I]; });
+    static_for<1, Q>([&](auto I) { anyface |= nb[I]; });
+    // scatter offsets within a component (S7, push): f*_i goes to the cell at x + e_i, or bounces into the own slot of plane ibar
+    const uint32_t cp = (uint32_t)p.cplane;
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
-        CT(&fk)[L::Q] = f[PARK ? 0 : k];
-        if constexpr (PARK) static_for<0, L::Q>([&](auto I) { fk[I] = park[(k * L::Q + I) * 128 + threadIdx.x]; });
+        CT fk[Q];
+        load_pops(k, fk);
         if constexpr (COLL != 2) collide<L, COLL, CT>(p, k, rho[k], u, du[k], fk);
         if (anyface & NBR_FACE) {   // a link of this cell crosses a non-periodic face: velocity / pressure rules (R10)
-            const int id = __ldg(p.flist + n);
-            if (__ldg(p.flags + id) & FACEBC_BIT) {
-                Cell cc;
-                cc.x = id % p.nx; cc.y = (id / p.nx) % p.ny; cc.z = id / (p.nx * p.ny);
-                apply_face_rules<L, CT>(p, cc, k, u, fk);
-            }
+            apply_face_rules_fn<L, CT>(p, [&](auto O) { return (nb[O] & NBR_FACE) ? (int)((nb[O] >> NBR_FACE_SHIFT) & 7u) : -1; }, k, u, fk);
         }
-        ST* out = static_cast<ST*>(p.f_out) + (long long)k * L::Q * p.cplane;
-        const uint32_t cp = (uint32_t)p.cplane;
-        static_for<0, L::Q>([&](auto I) { Conv<CT, ST>::st(out + ((uint32_t)I * cp + n), fk[I] - p.wref[I]); });
+        ST* out = static_cast<ST*>(p.f_out) + (long long)k * Q * p.cplane;
+        static_for<0, Q>([&](auto I) {
+            constexpr int i = I;
+            if constexpr (i == 0) {
+                Conv<CT, ST>::st(out + n, fk[0] - p.wref[0]);
+            } else {
+                constexpr int ib = opposite<L>(i);
+                const uint32_t d = nb[i];
+                const uint32_t off = d < (uint32_t)p.nfluid ? (uint32_t)i * cp + d : (uint32_t)ib * cp + n;
+                Conv<CT, ST>::st(out + off, fk[i] - p.wref[i]);   // (w_i = w_ibar)
+            }
+        });
     }
 }
 

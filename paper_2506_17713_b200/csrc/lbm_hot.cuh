@@ -619,15 +619,16 @@ __device__ __forceinline__ void force_and_velocity(const KParams<CT>& p, const C
 }
 
 // Links of a fluid cell that cross a velocity / pressure face: the rule is applied at the writing cell (R10), on the
-// post-collision populations fc of component k; uc = common velocity of the cell.
-template <class L, class CT>
-__device__ __forceinline__ void apply_face_rules(const KParams<CT>& p, const Cell& cc, int k, const CT (&uc)[3], CT (&fc)[L::Q]) {
+// post-collision populations fc of component k; uc = common velocity of the cell.  facefn(IC<o>) = the non-periodic face
+// the link along +e_o crosses, or -1.
+template <class L, class CT, class FaceFn>
+__device__ __forceinline__ void apply_face_rules_fn(const KParams<CT>& p, FaceFn&& facefn, int k, const CT (&uc)[3], CT (&fc)[L::Q]) {
     const CT uu15 = CT(1.5) * (uc[0] * uc[0] + uc[1] * uc[1] + uc[2] * uc[2]);
     static_for<1, L::Q>([&](auto O) {
         constexpr int o = O;
         constexpr int eox = L::E[o][0], eoy = L::E[o][1], eoz = L::E[o][2];
         constexpr CT w = CT(L::WN[o]) / CT(L::WD);
-        const int face = crossed_face<L, o>(p, cc);
+        const int face = facefn(O);
         if (face >= 0) {
             const int kind = p.face_kind[face];
             if (kind == FACE_VELOCITY) {   // arriving direction i = opposite(o), e_i = -e_o
@@ -645,6 +646,11 @@ __device__ __forceinline__ void apply_face_rules(const KParams<CT>& p, const Cel
             }
         }
     });
+}
+// ... with the face found from the cell's coordinates (dense layout)
+template <class L, class CT>
+__device__ __forceinline__ void apply_face_rules(const KParams<CT>& p, const Cell& cc, int k, const CT (&uc)[3], CT (&fc)[L::Q]) {
+    apply_face_rules_fn<L, CT>(p, [&](auto O) { return crossed_face<L, decltype(O)::value>(p, cc); }, k, uc, fc);
 }
 
 // ------------------------------------------------------------------ K1: rho + psi

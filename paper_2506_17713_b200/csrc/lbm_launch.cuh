@@ -11,7 +11,8 @@
 namespace lbmk {
 
 enum Op { OP_MOMENTS = 0, OP_VIRTUAL = 1, OP_STEP = 2, OP_INIT = 3, OP_EXPORT_MACRO = 4, OP_EXPORT_POP = 5, OP_IMPORT_POP = 6, OP_UNSTREAM = 7, OP_FUSED = 8,
-          OP_BUILD_NBR = 9 /* a0 = dense -> extended index map, a2 = table */, OP_FILL_SOLID = 10 };
+          OP_BUILD_NBR = 9 /* a0 = dense -> extended index map, a2 = table */, OP_FILL_SOLID = 10,
+          OP_PACK_C = 11 /* dense -> compact layout */, OP_UNPACK_C = 12 /* compact -> dense */ };
 
 struct LaunchArgs {
     int op;
@@ -148,7 +149,13 @@ cudaError_t launch(const LaunchArgs& a) {
                         }
                         if constexpr (B != 0) {
                             if (a.list == 2) {
-                                k_step_c<L, NC, CT, ST, C_><<<grid(p.nfluid, 128), 128, 0, a.stream>>>(p);
+                                using T = CompactTile<L, NC, ST>;
+                                auto kern = k_step_c<L, NC, CT, ST, C_>;
+                                if (T::SMEM > 48 * 1024) {
+                                    static bool optin = false;   // (per process; the attribute is sticky per device and function)
+                                    if (!optin) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM); optin = true; }
+                                }
+                                kern<<<grid(p.nfluid, T::CB), T::CB, T::SMEM, a.stream>>>(p);
                                 return;
                             }
                             if (a.list) {
@@ -169,6 +176,12 @@ cudaError_t launch(const LaunchArgs& a) {
             break;
         case OP_FILL_SOLID:
             with_nc([&](auto NC) { k_fill_solid<L, NC, CT, ST><<<grid(p.N, 256), 256, 0, a.stream>>>(p); });
+            break;
+        case OP_PACK_C:
+            with_nc([&](auto NC) { k_pack_c<L, NC, CT, ST><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p); });
+            break;
+        case OP_UNPACK_C:
+            with_nc([&](auto NC) { k_unpack_c<L, NC, CT, ST><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p); });
             break;
         case OP_UNSTREAM:
             with_nc([&](auto NC) {
