@@ -2,7 +2,7 @@
 //
 // With most cells solid (config 4: 77 %), the dense [cell] planes spend most of every 32-byte sector on solid slots that
 // nobody reads.  While lbm_step runs on such a domain the populations therefore live in the order of the fluid-cell list:
-// slot n of a direction plane belongs to the n-th fluid cell (ascending cell index; the planes are cplane = nfluid rounded
+// slot n of a direction plane belongs to the n-th fluid cell (brick order, lbm_api.cu; the planes are cplane = nfluid rounded
 // up to 64 elements apart, so the whole state is one contiguous block), and psi lives in "extended" order
 // (slots [0, nfluid) = fluid cells, [nfluid, nfluid + nbsolid) = boundary solids in the order of their list).
 // In this layout the planes hold the POST-STREAM populations f_i(x_n, t) ("push" streaming): K1 and K2 read nothing but
@@ -51,6 +51,51 @@ __global__ void __launch_bounds__(256) k_build_nbr(const __grid_constant__ KPara
         const uint32_t e = (uint32_t)__ldg(cmap + pc[0] + p.nx * (pc[1] + p.ny * pc[2]));
         nbr[(long long)(i - 1) * p.nbr_stride + n] = (e & NBR_IDX) | (face >= 0 ? NBR_FACE | ((uint32_t)face << NBR_FACE_SHIFT) : 0u);
     });
+}
+
+// per boundary solid: fluid-list index of each neighbour (0xffffffff: not fluid), from the dense -> extended index map
+template <class L, class CT>
+__global__ void __launch_bounds__(256) k_build_snbr(const __grid_constant__ KParams<CT> p, const int* __restrict__ cmap,
+                                                   uint32_t* __restrict__ snbr) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= p.nbsolid) return;
+    const int id = __ldg(p.bsolid + b);
+    const Cell c = make_cell<L>(p, id);
+    static_for<1, L::Q>([&](auto I) {
+        constexpr int i = I;
+        const uint32_t e = (uint32_t)__ldg(cmap + id + nbr_offset<L::E[i][0], L::E[i][1], L::E[i][2]>(c));
+        snbr[(long long)(i - 1) * p.snbr_stride + b] = e < (uint32_t)p.nfluid ? e : 0xffffffffu;
+    });
+}
+
+// K1b in compact order (S2, Eq. 17): rho of the fluid neighbours from the compact rho field K1 wrote (coalesced
+// table rows, gathers that stay in L2) instead of 18 scattered reads of the dense field; same operations in the same
+// order as k_virtual_density
+template <class L, int NC, class CT>
+__global__ void __launch_bounds__(128) k_virtual_density_c(const __grid_constant__ KParams<CT> p) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= p.nbsolid) return;
+    CT num[NC], den = CT(0);
+#pragma unroll
+    for (int k = 0; k < NC; ++k) num[k] = CT(0);
+    uint32_t e[L::Q];
+    static_for<1, L::Q>([&](auto I) { e[I] = __ldg(p.snbr + (long long)(I - 1) * p.snbr_stride + b); });
+    static_for<1, L::Q>([&](auto I) {
+        constexpr int i = I;
+        constexpr CT w = CT(L::WN[i]) / CT(L::WD);
+        if (e[i] != 0xffffffffu) {
+            den += w;
+#pragma unroll
+            for (int k = 0; k < NC; ++k) num[k] += w * __ldg(p.rho + (long long)k * p.N + e[i]);
+        }
+    });
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        CT rs = p.wet_phi[k] * (num[k] / den) - p.wet_drho[k];
+        rs = rs < p.wet_lo[k] ? p.wet_lo[k] : rs;
+        rs = rs > p.wet_hi[k] ? p.wet_hi[k] : rs;
+        p.psi[(long long)k * p.N + p.nfluid + b] = psi_of_rho(p, k, rs);
+    }
 }
 
 static __global__ void __launch_bounds__(256) k_cmap_scatter(int n, const int* __restrict__ list, int base, int* __restrict__ cmap) {
@@ -128,27 +173,31 @@ __device__ __forceinline__ void load_nbr(const KParams<CT>& p, unsigned n, uint3
 }
 
 // the Q populations that have arrived at fluid cell n: its own slot of every plane
-template <class L, class CT, class ST>
+template <class L, class CT, class ST, bool WREF>
 __device__ __forceinline__ void load_compact(const KParams<CT>& p, unsigned n, int k, CT (&f)[L::Q]) {
     // 32-bit element offsets within a component (Q * cplane < 2^32 is a condition of the mode)
     const ST* base = static_cast<const ST*>(p.f_in) + (long long)k * L::Q * p.cplane;
     const uint32_t cp = (uint32_t)p.cplane;
-    static_for<0, L::Q>([&](auto I) { f[I] = ld_one<CT, ST>(base + ((uint32_t)I * cp + n)) + p.wref[I]; });
+    static_for<0, L::Q>([&](auto I) {
+        f[I] = ld_one<CT, ST>(base + ((uint32_t)I * cp + n));
+        if constexpr (WREF) f[I] += p.wref[I];
+    });
 }
 
 // ------------------------------------------------------------------ K1 in compact order: a streaming read, no table
-template <class L, int NC, class CT, class ST>
+template <class L, int NC, class CT, class ST, bool WREF>
 __global__ void __launch_bounds__(256, 4) k_moments_c(const __grid_constant__ KParams<CT> p) {
     const unsigned n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= (unsigned)p.nfluid) return;
-    const int id = p.write_rho ? __ldg(p.flist + n) : 0;
+    // rho for K1b: in compact order when K1b has its neighbour table (snbr), else scattered into the dense field
+    const int id = !p.write_rho ? 0 : (p.snbr ? (int)n : __ldg(p.flist + n));
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
         CT f[L::Q];
-        load_compact<L, CT, ST>(p, n, k, f);
+        load_compact<L, CT, ST, WREF>(p, n, k, f);
         const CT r = density<L, CT>(f);
         p.psi[(long long)k * p.N + n] = psi_of_rho(p, k, r);
-        if (p.write_rho) p.rho[(long long)k * p.N + id] = r;   // dense: K1b averages it around the boundary solids
+        if (p.write_rho) p.rho[(long long)k * p.N + id] = r;
     }
 }
 
@@ -161,7 +210,8 @@ __global__ void __launch_bounds__(256, 4) k_moments_c(const __grid_constant__ KP
 // issued as soon as the copies have landed; several CTAs per SM hide that second round trip.
 template <class L, int NC, class ST>
 struct CompactTile {
-    static constexpr int CB = 128;                                  // cells per CTA = threads
+    static constexpr int CB = 256;                                  // cells per CTA = threads
+    static constexpr int CPW = (NC * L::Q + L::Q - 1 + CB / 32 - 1) / (CB / 32);   // copies issued per warp (its first lanes)
     static constexpr int NPOP = NC * L::Q;                          // population runs
     static constexpr int NTAB = L::Q - 1;                           // table rows
     static constexpr size_t POP_BYTES = (size_t)NPOP * CB * sizeof(ST);
@@ -169,8 +219,9 @@ struct CompactTile {
     static constexpr size_t SMEM = POP_BYTES + TAB_BYTES + 16;
 };
 
-template <class L, int NC, class CT, class ST, int COLL>
-__global__ void __launch_bounds__(128, (sizeof(ST) == 2 ? 8 : 6)) k_step_c(const __grid_constant__ KParams<CT> p) {
+// WREF: populations are stored shifted by w_i rho_ref (R16)
+template <class L, int NC, class CT, class ST, int COLL, bool WREF>
+__global__ void __launch_bounds__(256, (sizeof(ST) == 2 ? 4 : 3)) k_step_c(const __grid_constant__ KParams<CT> p) {
     using T = CompactTile<L, NC, ST>;
     constexpr int Q = L::Q, CB = T::CB;
     extern __shared__ __align__(16) unsigned char smem_c[];
@@ -189,13 +240,14 @@ __global__ void __launch_bounds__(128, (sizeof(ST) == 2 ? 8 : 6)) k_step_c(const
     __syncthreads();
     if (t == 0) mbar_expect_tx(bar, cnt * (uint32_t)(T::NPOP * sizeof(ST) + T::NTAB * 4));
     __syncthreads();
-    if (t < T::NPOP) {
-        const int k = t / Q, i = t - k * Q;
-        const ST* src = static_cast<const ST*>(p.f_in) + ((long long)k * Q * p.cplane + (long long)i * p.cplane + n0);
-        bulk_g2s(pops + t * CB, src, cnt * (uint32_t)sizeof(ST), bar);
-    } else if (t < T::NPOP + T::NTAB) {
-        const int i = t - T::NPOP;
-        bulk_g2s(tab + i * CB, p.nbr + ((long long)i * p.nbr_stride + n0), cnt * 4u, bar);
+    {   // every warp issues CPW of the NPOP + NTAB copies (the issue loop is serial within a warp)
+        const int lane = t & 31, c = (int)(t >> 5) * T::CPW + lane;
+        if (lane < T::CPW && c < T::NPOP) {
+            bulk_g2s(pops + c * CB, static_cast<const ST*>(p.f_in) + ((long long)c * p.cplane + n0), cnt * (uint32_t)sizeof(ST), bar);
+        } else if (lane < T::CPW && c < T::NPOP + T::NTAB) {
+            const int i = c - T::NPOP;
+            bulk_g2s(tab + i * CB, p.nbr + ((long long)i * p.nbr_stride + n0), cnt * 4u, bar);
+        }
     }
     mbar_wait(bar, 0);
     if (n >= (unsigned)p.nfluid) return;
@@ -229,7 +281,10 @@ __global__ void __launch_bounds__(128, (sizeof(ST) == 2 ? 8 : 6)) k_step_c(const
         }
     }
     auto load_pops = [&](int k, CT (&fk)[Q]) {
-        static_for<0, Q>([&](auto I) { fk[I] = Cvt<CT, ST>::up(pops[(k * Q + I) * CB + t]) + p.wref[I]; });
+        static_for<0, Q>([&](auto I) {
+            fk[I] = Cvt<CT, ST>::up(pops[(k * Q + I) * CB + t]);
+            if constexpr (WREF) fk[I] += p.wref[I];
+        });
     };
     CT rho[NC], j[NC][3];
     CT u[3] = {CT(0), CT(0), CT(0)}, du[NC][3];
@@ -258,12 +313,12 @@ __global__ void __launch_bounds__(128, (sizeof(ST) == 2 ? 8 : 6)) k_step_c(const
         static_for<0, Q>([&](auto I) {
             constexpr int i = I;
             if constexpr (i == 0) {
-                Conv<CT, ST>::st(out + n, fk[0] - p.wref[0]);
+                Conv<CT, ST>::st(out + n, WREF ? fk[0] - p.wref[0] : fk[0]);
             } else {
                 constexpr int ib = opposite<L>(i);
                 const uint32_t d = nb[i];
                 const uint32_t off = d < (uint32_t)p.nfluid ? (uint32_t)i * cp + d : (uint32_t)ib * cp + n;
-                Conv<CT, ST>::st(out + off, fk[i] - p.wref[i]);   // (w_i = w_ibar)
+                Conv<CT, ST>::st(out + off, WREF ? fk[i] - p.wref[i] : fk[i]);   // (w_i = w_ibar)
             }
         });
     }

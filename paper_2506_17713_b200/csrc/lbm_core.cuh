@@ -134,13 +134,15 @@ struct KParams {
     const int* bsolid; // boundary-solid list
     int nbsolid;
     const uint32_t* bmask;  // per boundary solid: bit i <=> the neighbour at x + e_i is fluid (NULL: test the flags)
-    const int* flist;  // fluid-cell list, ascending (list mode of the hot kernels on porous domains)
+    const int* flist;  // fluid-cell list in brick order (lbm_api.cu VisitOrder; list / compact mode of the hot kernels)
     int nfluid;
     // compact mode (lbm_compact.cuh): neighbour table [(Q-1)][nbr_stride] of extended indices; psi in extended order
     const uint32_t* nbr;
     long long nbr_stride;
     long long cplane;   // elements between consecutive direction planes in compact order (= nbr_stride)
     int compact;
+    const uint32_t* snbr;   // compact mode: per boundary solid, the fluid-list index of the cell at x_s + e_i or 0xffffffff: [(Q-1)][snbr_stride]
+    long long snbr_stride;  // (NULL: K1b gathers the dense rho field through cell coordinates)
     // mode
     int forcing;       // 0 EDM, 1 SHIFT
     int write_rho;     // K1 also writes rho (needed by K1b and the exports)

@@ -12,7 +12,8 @@ namespace lbmk {
 
 enum Op { OP_MOMENTS = 0, OP_VIRTUAL = 1, OP_STEP = 2, OP_INIT = 3, OP_EXPORT_MACRO = 4, OP_EXPORT_POP = 5, OP_IMPORT_POP = 6, OP_UNSTREAM = 7, OP_FUSED = 8,
           OP_BUILD_NBR = 9 /* a0 = dense -> extended index map, a2 = table */, OP_FILL_SOLID = 10,
-          OP_PACK_C = 11 /* dense -> compact layout */, OP_UNPACK_C = 12 /* compact -> dense */ };
+          OP_PACK_C = 11 /* dense -> compact layout */, OP_UNPACK_C = 12 /* compact -> dense */,
+          OP_BUILD_SNBR = 13 /* a0 = dense -> extended index map, a2 = table of the boundary solids */ };
 
 struct LaunchArgs {
     int op;
@@ -112,7 +113,8 @@ cudaError_t launch(const LaunchArgs& a) {
                     constexpr int VW = vec_width<CT, ST, NC>();
                     if constexpr (B != 0) {
                         if (a.list == 2) {
-                            k_moments_c<L, NC, CT, ST><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p);
+                            if (a.wref) k_moments_c<L, NC, CT, ST, true><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p);
+                            else k_moments_c<L, NC, CT, ST, false><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p);
                             return;
                         }
                         if (a.list) {
@@ -129,7 +131,10 @@ cudaError_t launch(const LaunchArgs& a) {
             break;
         case OP_VIRTUAL:
             if (p.nbsolid > 0)
-                with_nc([&](auto NC) { launch_hot(k_virtual_density<L, NC, CT>, grid(p.nbsolid, 128), 128); });
+                with_nc([&](auto NC) {
+                    if (p.compact && p.snbr) k_virtual_density_c<L, NC, CT><<<grid(p.nbsolid, 128), 128, 0, a.stream>>>(p);
+                    else launch_hot(k_virtual_density<L, NC, CT>, grid(p.nbsolid, 128), 128);
+                });
             break;
         case OP_STEP:
             with_nc([&](auto NC) {
@@ -150,12 +155,12 @@ cudaError_t launch(const LaunchArgs& a) {
                         if constexpr (B != 0) {
                             if (a.list == 2) {
                                 using T = CompactTile<L, NC, ST>;
-                                auto kern = k_step_c<L, NC, CT, ST, C_>;
-                                if (T::SMEM > 48 * 1024) {
-                                    static bool optin = false;   // (per process; the attribute is sticky per device and function)
-                                    if (!optin) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM); optin = true; }
-                                }
-                                kern<<<grid(p.nfluid, T::CB), T::CB, T::SMEM, a.stream>>>(p);
+                                auto go_c = [&](auto kern) {
+                                    if (T::SMEM > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM);
+                                    kern<<<grid(p.nfluid, T::CB), T::CB, T::SMEM, a.stream>>>(p);
+                                };
+                                if (a.wref) go_c(k_step_c<L, NC, CT, ST, C_, true>);
+                                else go_c(k_step_c<L, NC, CT, ST, C_, false>);
                                 return;
                             }
                             if (a.list) {
@@ -173,6 +178,9 @@ cudaError_t launch(const LaunchArgs& a) {
             break;
         case OP_BUILD_NBR:
             k_build_nbr<L, CT><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p, static_cast<const int*>(a.a0), static_cast<uint32_t*>(a.a2));
+            break;
+        case OP_BUILD_SNBR:
+            k_build_snbr<L, CT><<<grid(p.nbsolid, 256), 256, 0, a.stream>>>(p, static_cast<const int*>(a.a0), static_cast<uint32_t*>(a.a2));
             break;
         case OP_FILL_SOLID:
             with_nc([&](auto NC) { k_fill_solid<L, NC, CT, ST><<<grid(p.N, 256), 256, 0, a.stream>>>(p); });
