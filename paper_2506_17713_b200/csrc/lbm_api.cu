@@ -806,15 +806,15 @@ int prepare(lbm* h) {
             h->nbsolid = cnt[0];
             h->nfluid = cnt[1];
             if (h->nbsolid > 0) {
-                // the atomic append left the boundary solids in arbitrary order: rewrite the list in ascending cell order
-                // (deterministic; neighbouring threads of K1b, and the psi gathers of the compact mode, then touch
-                // neighbouring memory).  Scratch: the rho field (zeroed again below).
+                // the atomic append left the boundary solids in arbitrary order: rewrite the list in the brick order of the
+                // fluid list (deterministic; neighbouring threads of K1b, and the psi gathers of the compact mode, then
+                // touch neighbouring memory; lbm_get_boundary_solids sorts its copy).  Scratch: the rho field (zeroed below).
                 uint32_t* marks = reinterpret_cast<uint32_t*>(h->ws + h->cv.rho);
                 CU(cudaMemsetAsync(marks, 0, (size_t)h->N * 4, h->stream));
                 k_mark<<<(h->nbsolid + 255) / 256, 256, 0, h->stream>>>(h->nbsolid, list, marks);
-                k_fluid_count<<<nb, COMPACT_BLOCK, 0, h->stream>>>(plain, marks, blockcnt, 1u, 1u);
-                k_fluid_scan<<<1, 1024, 0, h->stream>>>(nb, blockcnt);
-                k_fluid_fill<<<nb, COMPACT_BLOCK, 0, h->stream>>>(plain, marks, blockcnt, list, 1u, 1u);
+                k_fluid_count<<<nbf, COMPACT_BLOCK, 0, h->stream>>>(vo, marks, blockcnt, 1u, 1u);
+                k_fluid_scan<<<1, 1024, 0, h->stream>>>(nbf, blockcnt);
+                k_fluid_fill<<<nbf, COMPACT_BLOCK, 0, h->stream>>>(vo, marks, blockcnt, list, 1u, 1u);
                 CU(cudaGetLastError());
                 h->launches += 4;
                 CU(cudaMemsetAsync(h->ws + h->cv.rho, 0, (size_t)h->cfg.n_components * h->N * h->cbytes, h->stream));

@@ -210,7 +210,10 @@ __global__ void __launch_bounds__(256, 4) k_moments_c(const __grid_constant__ KP
 // issued as soon as the copies have landed; several CTAs per SM hide that second round trip.
 template <class L, int NC, class ST>
 struct CompactTile {
-    static constexpr int CB = 256;                                  // cells per CTA = threads
+    // cells per CTA = threads, CTAs per SM (measured on config 4, K2: fp32 store 256 x 3 1.18 ms, 128 x 7 1.27, 128 x 8 1.42;
+    // fp16 store 128 x 7 0.89 ms, 256 x 3 1.04)
+    static constexpr int CB = sizeof(ST) == 2 ? 128 : 256;
+    static constexpr int CTAS = sizeof(ST) == 2 ? 7 : 3;
     static constexpr int CPW = (NC * L::Q + L::Q - 1 + CB / 32 - 1) / (CB / 32);   // copies issued per warp (its first lanes)
     static constexpr int NPOP = NC * L::Q;                          // population runs
     static constexpr int NTAB = L::Q - 1;                           // table rows
@@ -221,7 +224,7 @@ struct CompactTile {
 
 // WREF: populations are stored shifted by w_i rho_ref (R16)
 template <class L, int NC, class CT, class ST, int COLL, bool WREF>
-__global__ void __launch_bounds__(256, (sizeof(ST) == 2 ? 4 : 3)) k_step_c(const __grid_constant__ KParams<CT> p) {
+__global__ void __launch_bounds__((CompactTile<L, NC, ST>::CB), (CompactTile<L, NC, ST>::CTAS)) k_step_c(const __grid_constant__ KParams<CT> p) {
     using T = CompactTile<L, NC, ST>;
     constexpr int Q = L::Q, CB = T::CB;
     extern __shared__ __align__(16) unsigned char smem_c[];
