@@ -87,10 +87,17 @@ enum lbm_face_kind { LBM_FACE_PERIODIC = 0, LBM_FACE_WALL = 1, LBM_FACE_VELOCITY
 /* flags */
 #define LBM_FLAG_NO_COLLIDE 1u /* f* = f: pure streaming, for the bit-exact permutation test */
 #define LBM_FLAG_TWO_PASS 2u   /* always run the two-pass path K1 (+K1b) + K2 */
-#define LBM_FLAG_ONE_PASS 4u   /* require the one-pass kernel K2F: lbm_step fails with LBM_E_UNSUPPORTED where it does not
-                                  apply (solid cells, a non-periodic axis, nx not a multiple of the vector width, or a
-                                  dtype/component combination it is not built for).  Default (neither flag): K2F where it
-                                  applies and the domain is large enough to fill the GPU, else two-pass. */
+#define LBM_FLAG_ONE_PASS 4u   /* require a one-pass kernel K2F: lbm_step fails with LBM_E_UNSUPPORTED where none applies
+                                  (D2Q9, solid cells, a non-periodic axis, rows that are not whole 16-byte vectors of the
+                                  storage dtype, or a dtype/component combination it is not built for).  Default (neither
+                                  flag): K2F where it applies and the domain is large enough to fill the GPU, else two-pass. */
+
+/* Tuning knobs.  NOT part of the ABI: environment variables read once, in lbm_create, for measurements and tests; no other
+ * call reads the environment.  LBM_TUNE_FUSED_MCHUNK=<planes marched per CTA of the one-pass kernels>, LBM_TUNE_NO_EQ (run
+ * k_fused_ws where k_fused_eq would apply), LBM_TUNE_EQ_HALF=0|1 (tile width of k_fused_eq), LBM_TUNE_LIST=0|1 and
+ * LBM_TUNE_COMPACT=0 (list / fluid-compact mode of the two-pass path on masked domains), LBM_TUNE_BRICK="bx,by,bz" (order of
+ * the fluid-cell list), LBM_TUNE_NO_SNBR, LBM_TUNE_NO_PDL / LBM_TUNE_NO_GRAPH / LBM_TUNE_NO_COOP (plain launches on small
+ * domains).  Results never depend on them beyond rounding order (none changes any arithmetic). */
 
 typedef struct {
     int32_t psi_kind; /* lbm_psi_kind */
@@ -156,8 +163,11 @@ LBM_API int lbm_set_solid_mask(lbm_t* h, const uint8_t* mask, int on_device);
 
 /* Boundary condition of one face of a non-periodic axis (reading R10): LBM_FACE_WALL (halfway
  * bounce-back), LBM_FACE_VELOCITY (bounce-back + 2 w_i rho_w e_i.u_w/c_s^2) or LBM_FACE_PRESSURE
- * (anti-bounce-back with rho_w; velocity = the boundary node's own).  rho_w[2] per component,
- * u_w[3].  LBM_E_INVALID for a face of a periodic axis. */
+ * (anti-bounce-back f_i = -f*_ibar + 2 w_i rho_w [1 + (e_i.u)^2/(2 c_s^4) - u.u/(2 c_s^2)] with the boundary node's own
+ * velocity u: the one bracket for which a uniform equilibrium flow passes the face unchanged).  rho_w[2] per component,
+ * u_w[3].  LBM_E_INVALID for a face of a periodic axis.  The rule is folded into the stored populations at the writing
+ * cell, so a face can be (re)defined before lbm_init_fields or between lbm_init_fields and the first lbm_step only:
+ * LBM_E_STATE once steps have run (call lbm_init_fields again to start over). */
 LBM_API int lbm_set_face_bc(lbm_t* h, int face, int kind, const double* rho_w, const double* u_w);
 
 /* S0: f_i^k = f_eq,i(rho^k, u) at fluid cells (solid cells hold f_eq(1,0) and are never updated);
@@ -165,7 +175,9 @@ LBM_API int lbm_set_face_bc(lbm_t* h, int face, int kind, const double* rho_w, c
  * element type of the arrays. */
 LBM_API int lbm_init_fields(lbm_t* h, const void* const* rho, const void* u, int dtype, int on_device);
 
-/* Enqueue n >= 0 time steps (S1..S7) on the stream.  Asynchronous; no host synchronisation.
+/* Enqueue n >= 0 time steps (S1..S7) on the stream.  Asynchronous; no host synchronisation -- with one exception: on a
+ * domain with a solid mask, the first lbm_init_fields / lbm_step / export after lbm_set_solid_mask or lbm_set_face_bc
+ * builds the link flags and cell lists and reads two counters back (one stream synchronisation, once per mask).
  * Layout note: on a masked domain with at most a quarter of the cells fluid (and a plain Shan-Chen force) the steps
  * run on a fluid-compact copy of the populations (lbm_hot_path reports LBM_PATH_TWO_PASS_COMPACT); the first step
  * after, and the first export / import after such steps, each cost one extra copy kernel.  Results are bit-identical
@@ -233,7 +245,7 @@ LBM_API int lbm_get_kernel_times(lbm_t* h, double* ms_total, int64_t* launches);
 enum lbm_path {
     LBM_PATH_NONE = 0,              /* no step yet */
     LBM_PATH_TWO_PASS = 1,          /* K1 (+K1b) + K2 */
-    LBM_PATH_ONE_PASS_LOCKSTEP = 2, /* K2F k_fused_v */
+    LBM_PATH_RESERVED_2 = 2,        /* (round 1's lock-step one-pass kernel; removed) */
     LBM_PATH_ONE_PASS_WS = 3,       /* K2F k_fused_ws (warp-specialised, bulk asynchronous copies) */
     LBM_PATH_TWO_PASS_COMPACT = 4,  /* K1 (+K1b) + K2 on the fluid-compact layout (at most a quarter of the cells fluid) */
     LBM_PATH_ONE_PASS_EQ = 5        /* K2F k_fused_eq (row pipelines; one component, BGK with tau = 1) */

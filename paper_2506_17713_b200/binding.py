@@ -355,10 +355,8 @@ class LBM:
 
     @property
     def hot_path(self) -> str:
-        """What the most recent step() launched: 'two_pass', 'one_pass_lockstep', 'one_pass_ws', 'one_pass_eq' or
-        'two_pass_compact'."""
-        return {0: "none", 1: "two_pass", 2: "one_pass_lockstep", 3: "one_pass_ws", 4: "two_pass_compact",
-                5: "one_pass_eq"}[int(self.L.lbm_hot_path(self.h))]
+        """What the most recent step() launched: 'two_pass', 'one_pass_ws', 'one_pass_eq' or 'two_pass_compact'."""
+        return {0: "none", 1: "two_pass", 3: "one_pass_ws", 4: "two_pass_compact", 5: "one_pass_eq"}[int(self.L.lbm_hot_path(self.h))]
 
     @property
     def steps_done(self) -> int:

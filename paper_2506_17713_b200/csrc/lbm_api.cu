@@ -29,8 +29,41 @@ struct Carve {
 
 }  // namespace
 
+// Tuning knobs: environment variables read ONCE, in lbm_create (include/lbm.h lists them; not part of the ABI)
+struct Tune {
+    int mchunk = 0;        // LBM_TUNE_FUSED_MCHUNK: planes marched per CTA of the one-pass kernels (0 = cost model)
+    int list = -1;         // LBM_TUNE_LIST: force list mode on (1) / off (0)
+    int compact = -1;      // LBM_TUNE_COMPACT=0: keep the dense layout where compact mode would apply
+    int eq = -1;           // LBM_TUNE_NO_EQ=1 -> 0: k_fused_ws where k_fused_eq would apply
+    int eq_half = -1;      // LBM_TUNE_EQ_HALF: force full-width (0) / half-width (1) tiles of k_fused_eq
+    bool no_snbr = false;  // LBM_TUNE_NO_SNBR: K1b of the compact mode on the dense rho field
+    bool no_pdl = false;   // LBM_TUNE_NO_PDL / LBM_TUNE_NO_GRAPH / LBM_TUNE_NO_COOP: plain launches on small domains
+    bool no_graph = false;
+    bool no_coop = false;
+    int brick[3] = {32, 16, 16};   // LBM_TUNE_BRICK="bx,by,bz": bricks of the fluid list's order (bx = 0: ascending cell index)
+    static Tune from_env() {
+        Tune t;
+        auto geti = [](const char* name, int dflt) { const char* e = std::getenv(name); return e ? std::atoi(e) : dflt; };
+        t.mchunk = geti("LBM_TUNE_FUSED_MCHUNK", 0);
+        t.list = geti("LBM_TUNE_LIST", -1);
+        t.compact = geti("LBM_TUNE_COMPACT", -1);
+        t.eq = std::getenv("LBM_TUNE_NO_EQ") ? 0 : -1;
+        t.eq_half = geti("LBM_TUNE_EQ_HALF", -1);
+        t.no_snbr = std::getenv("LBM_TUNE_NO_SNBR") != nullptr;
+        t.no_pdl = std::getenv("LBM_TUNE_NO_PDL") != nullptr;
+        t.no_graph = std::getenv("LBM_TUNE_NO_GRAPH") != nullptr;
+        t.no_coop = std::getenv("LBM_TUNE_NO_COOP") != nullptr;
+        if (const char* e = std::getenv("LBM_TUNE_BRICK")) {
+            int v[3] = {0, 1, 1};
+            if (std::sscanf(e, "%d,%d,%d", &v[0], &v[1], &v[2]) >= 1) { t.brick[0] = v[0]; t.brick[1] = std::max(1, v[1]); t.brick[2] = std::max(1, v[2]); }
+        }
+        return t;
+    }
+};
+
 struct lbm {
     lbm_config_t cfg;
+    Tune tune;
     int q, d, N;
     long long plane;
     size_t sbytes, cbytes;
@@ -40,7 +73,6 @@ struct lbm {
     int cur;
     int vec;   // cells per thread in the hot kernels (1 or the dtype's vector width)
     FusedShape fshape;   // tile of the one-pass kernel K2F (vec = 0: not built for this configuration)
-    int fvariant;        // tuning variant of K2F (0 = default)
     int fmchunk;         // planes marched per CTA
     bool use_fused;      // decided in prepare()
     bool eq_half;        // k_fused_eq with half-width tiles and two CTAs per SM
@@ -116,20 +148,14 @@ int check_config(const lbm_config_t* c) {
     return LBM_OK;
 }
 
-// bricks of the fluid-cell list's visit order (VisitOrder in the preprocessing kernels): 32 x 16 x 16 cells (32 x 16 on D2Q9)
-void brick_dims(const lbm_config_t& c, int (&b)[3]) {
-    b[0] = 32; b[1] = 16; b[2] = c.nz > 1 ? 16 : 1;   // (measured on config 4, K2: plain 1.45 ms, 16x4x4 1.40, 8x8x8 1.34, 16x8x8 1.29, 32x16x16 1.22, 32^3 1.20)
-    if (const char* e = std::getenv("LBM_TUNE_BRICK")) {   // "bx,by,bz"; bx = 0: plain ascending order
-        int v[3] = {0, 1, 1};
-        if (std::sscanf(e, "%d,%d,%d", &v[0], &v[1], &v[2]) >= 1) { b[0] = v[0]; b[1] = std::max(1, v[1]); b[2] = c.nz > 1 ? std::max(1, v[2]) : 1; }
-    }
-}
-long long brick_volume(const lbm_config_t& c) {   // positions the blocked order visits (brick-padded domain)
-    int b[3];
-    brick_dims(c, b);
+// Bricks of the fluid-cell list's visit order (VisitOrder in the preprocessing kernels): 32 x 16 x 16 cells by default
+// (measured on config 4, K2: ascending cell order 1.45 ms, 16x4x4 1.40, 8x8x8 1.34, 16x8x8 1.29, 32x16x16 1.22, 32^3 1.20);
+// every dimension is at most BRICK_MAX, which is what the workspace is sized for.
+constexpr int BRICK_MAX = 64;
+long long brick_volume(const lbm_config_t& c, const int (&b)[3]) {   // positions the brick order visits (brick-padded domain)
     if (b[0] <= 0) return (long long)c.nx * c.ny * c.nz;
     auto up = [](long long n, int m) { return (n + m - 1) / m * m; };
-    return up(c.nx, b[0]) * up(c.ny, b[1]) * up(c.nz, b[2]);
+    return up(c.nx, b[0]) * up(c.ny, b[1]) * up(c.nz, c.nz > 1 ? b[2] : 1);
 }
 
 Carve carve(const lbm_config_t& c) {
@@ -146,7 +172,8 @@ Carve carve(const lbm_config_t& c) {
     v.rho = take(nc * N * cb);
     v.flags = take(N * 4);
     v.bsolid = take(N * 4);
-    const size_t npos = (size_t)std::max<long long>((long long)N, brick_volume(c));
+    const int bmax[3] = {BRICK_MAX, BRICK_MAX, BRICK_MAX};
+    const size_t npos = (size_t)std::max<long long>((long long)N, brick_volume(c, bmax));
     v.flist = take(N * 4 + ((npos + 1023) / 1024 + 1) * 4);   // fluid-cell list + per-block counts of its compaction
     v.nbr = take((q - 1) * (N / 4 + 64) * 4);   // neighbour table of the compact mode (fluid fraction <= 1/4)
     v.snbr = take((q - 1) * (N / 4 + 64) * 4);  // ... and of its boundary solids (used when there are at most N/4 of them)
@@ -610,13 +637,10 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.zc = (zc && op == OP_STEP && !(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) ? 1 : 0;
     a.list = (h->use_list && (op == OP_MOMENTS || (op == OP_STEP && !a.zc))) ? (h->is_compact ? 2 : 1) : 0;
     a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
-    a.variant = h->fvariant;
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;   // (also read by the compact kernels)
-    a.pfd = 0;
     a.eq = h->feq ? (h->eq_half ? 2 : 1) : 0;
     a.pdl = h->pdl ? 1 : 0;
     a.used_kernel = op == OP_FUSED ? &h->last_path : nullptr;
-    if (const char* e = std::getenv("LBM_TUNE_FUSED_PFD")) a.pfd = std::atoi(e);
     a.stream = h->stream;
     launch_fn fn = pick_launch(h->cfg);
     if (!fn) return fail(h, LBM_E_UNSUPPORTED, "dtype combination not built");
@@ -660,26 +684,11 @@ static_assert(sizeof(FieldIOAny) == sizeof(FieldIO<float>) && sizeof(FieldIOAny)
               "FieldIO layout");
 
 // shape of K2F built for this configuration (mirrors the template dispatch in lbm_launch.cuh)
-FusedShape fused_shape_of(const lbm_config_t& c, int variant) {
-    FusedShape none{0, 0, 0};
-    auto pick = [&](auto L) -> FusedShape {
-        using LT = decltype(L);
-        const bool f32 = c.compute_dtype == LBM_F32;
-        if (variant == 13) {   // tuning: k_fused_ws with half-width tiles and four stages
-            if (LT::D == 3 && c.n_components == 1 && f32) return FusedShape{2, 1, 8};
-            return none;
-        }
-        if (variant > 0) {
-#ifdef LBM_FUSED_TUNING
-            if (LT::D == 3 && f32 && c.n_components == 1 && c.collision == LBM_BGK && variant <= FUSED_TUNING_VARIANTS)
-                return fused_tuning_shape(variant);
-#endif
-            return none;
-        }
-        if (f32) return c.n_components == 1 ? fused_shape<LT, float, float, 1>() : fused_shape<LT, float, float, 2>();
-        return c.n_components == 1 ? fused_shape<LT, double, double, 1>() : fused_shape<LT, double, double, 2>();
-    };
-    return c.lattice == LBM_D2Q9 ? pick(D2Q9{}) : pick(D3Q19{});
+FusedShape fused_shape_of(const lbm_config_t& c) {
+    if (c.lattice != LBM_D3Q19) return FusedShape{0, 0};
+    const bool f32 = c.compute_dtype == LBM_F32;
+    if (f32) return c.n_components == 1 ? fused_shape<D3Q19, float, float, 1>() : fused_shape<D3Q19, float, float, 2>();
+    return c.n_components == 1 ? fused_shape<D3Q19, double, double, 1>() : fused_shape<D3Q19, double, double, 2>();
 }
 
 // Does the one-pass kernel apply, and how many planes does a CTA march?  Fully periodic, no solid cells, collision on.
@@ -690,33 +699,32 @@ void plan_fused(lbm* h) {
     if (c.flags & (LBM_FLAG_TWO_PASS | LBM_FLAG_NO_COLLIDE)) return;
     if (c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0)))
         return;   // Zhang-Chen weight / surface-tension source: two-pass path
-    if (h->bnd || h->fshape.vec == 0 || c.nx % h->fshape.vec != 0) return;
+    // D3Q19 only, rows that are whole 16-byte vectors of the storage dtype (the bulk copies carry 16-byte pads)
+    if (h->bnd || h->fshape.vec == 0 || c.nx % h->fshape.vec != 0 || c.nx % (16 / (int)h->sbytes) != 0) return;
     if ((unsigned long long)c.n_components * h->q * (unsigned long long)h->plane >= (1ULL << 32)) return;   // 32-bit element offsets
-    if (h->d == 3 && c.nx % (16 / (int)h->sbytes) != 0 && h->fvariant == 0) h->fvariant = -1;   // k_fused_ws copies 16-byte pads
-    const int nm = h->d == 3 ? c.nz : c.ny;
+    const int nm = c.nz;
+    int nsm = 148, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);   // the device the handle was created on
     // k_fused_eq: one component, BGK, tau = 1
-    h->feq = h->d == 3 && h->fvariant == 0 && c.n_components == 1 && c.collision == LBM_BGK && c.tau[0] == 1.0 &&
-             !std::getenv("LBM_TUNE_NO_EQ");
+    h->feq = c.n_components == 1 && c.collision == LBM_BGK && c.tau[0] == 1.0 && h->tune.eq != 0;
     // half-width tiles, two CTAs per SM: where a full-width last tile would leave more than a tenth of the row's lanes idle
     // and half-width tiles fewer, or where full-width tiles cannot give every SM a column (measured: 416^3 2.67 -> 2.59 ms,
     // 128^3 0.0756 -> 0.0733; 512^3 3.9 -> 4.85: full width there)
     {
-        const int txf = h->fshape.wx * 32 * h->fshape.vec, txh = txf / 2;
+        const int txf = 32 * h->fshape.vec, txh = txf / 2;
         const double uf = (double)c.nx / (((c.nx + txf - 1) / txf) * (double)txf), uh = (double)c.nx / (((c.nx + txh - 1) / txh) * (double)txh);
         const long long cols = (long long)((c.nx + txf - 1) / txf) * ((c.ny + h->fshape.ty - 1) / h->fshape.ty);
-        int nsm0 = 148;
-        cudaDeviceGetAttribute(&nsm0, cudaDevAttrMultiProcessorCount, 0);
-        if (!std::getenv("LBM_TUNE_EQ_HALF")) h->eq_half = h->fshape.vec >= 2 && ((uf < 0.9 && uh > uf + 0.05) || cols < nsm0 / 4);
+        h->eq_half = h->tune.eq_half >= 0 ? h->tune.eq_half != 0
+                                          : h->fshape.vec >= 2 && ((uf < 0.9 && uh > uf + 0.05) || cols < nsm / 4);
     }
     const bool half = h->feq && h->eq_half;
-    const int tx = h->fshape.wx * 32 * h->fshape.vec / (half ? 2 : 1);
+    const int tx = 32 * h->fshape.vec / (half ? 2 : 1);
     const int ty = h->fshape.ty;
     const long long tiles = (long long)((c.nx + tx - 1) / tx) * (h->d == 3 ? (c.ny + ty - 1) / ty : 1);
     // Chunks per column of tiles: every CTA pulls two extra planes and pays a few planes' worth of pipeline fill, and
     // CTAs run in waves of one per SM, so minimise  waves * (planes per chunk + 5)  (measured on 128^3 .. 512^3: the
     // model picks 16, 128 and 128 planes, the best of the sweeps in DESIGN.md 6)
-    int nsm = 148;
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
     const long long slots = (long long)nsm * (half ? 2 : 1);   // CTAs resident at a time
     long long best_cost = -1;
     int mchunk = nm;
@@ -726,18 +734,14 @@ void plan_fused(lbm* h) {
         const long long cost = ((ctas + slots - 1) / slots) * (mc + 5);
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; mchunk = mc; }
     }
-    if (const char* e = std::getenv("LBM_TUNE_FUSED_MCHUNK")) mchunk = std::max(1, std::min(nm, std::atoi(e)));
+    if (h->tune.mchunk > 0) mchunk = std::max(1, std::min(nm, h->tune.mchunk));
     h->fmchunk = mchunk;
     // small domains cannot fill the GPU with marching CTAs: keep the two-pass path unless K2F is demanded
     const long long ctas = tiles * ((nm + mchunk - 1) / mchunk);
     // ... and rows that leave more than a fifth of the lanes of the last x tile idle (measured: 96^3, 192^3 no gain)
     const int xt = (c.nx + tx - 1) / tx;
     const bool lanes_ok = 5 * c.nx >= 4 * xt * tx;
-    // By default only the warp-specialised kernel counts (D3Q19): the lock-step kernel (D2Q9, and D3Q19 rows that are not
-    // whole 16-byte vectors) is slower than the two-pass path (measured: D2Q9 4096^2 29 against 57 GMLUPS) and runs on
-    // demand only.
-    const bool ws = h->d == 3 && h->fvariant != -1;
-    h->use_fused = (c.flags & LBM_FLAG_ONE_PASS) || (ws && 4 * ctas >= 3LL * nsm && lanes_ok);
+    h->use_fused = (c.flags & LBM_FLAG_ONE_PASS) || (4 * ctas >= 3LL * nsm && lanes_ok);
 }
 
 Geo make_geo(const lbm* h) {
@@ -784,9 +788,9 @@ int prepare(lbm* h) {
             const VisitOrder plain{h->cfg.nx, h->cfg.ny, h->cfg.nz, 0, 1, 1, 1, 1, (long long)h->N};
             VisitOrder vo = plain;                      // the fluid-cell list is brick-ordered (VisitOrder)
             {
-                int b[3];
-                brick_dims(h->cfg, b);
-                const long long vol = brick_volume(h->cfg);
+                int b[3] = {std::min(h->tune.brick[0], BRICK_MAX), std::min(h->tune.brick[1], BRICK_MAX),
+                            h->cfg.nz > 1 ? std::min(h->tune.brick[2], BRICK_MAX) : 1};
+                const long long vol = brick_volume(h->cfg, b);
                 if (b[0] > 0 && vol < (1LL << 31)) {
                     vo.bx = b[0]; vo.by = b[1]; vo.bz = b[2];
                     vo.nbx = (h->cfg.nx + b[0] - 1) / b[0]; vo.nby = (h->cfg.ny + b[1] - 1) / b[1];
@@ -830,7 +834,7 @@ int prepare(lbm* h) {
             }
             // with most cells solid the dense mapping wastes lanes and issue slots on them: one thread per fluid cell
             h->use_list = h->nfluid > 0 && h->nfluid < h->N / 2;   // (an all-solid domain has nothing to list)
-            if (const char* e = std::getenv("LBM_TUNE_LIST")) h->use_list = h->nfluid > 0 && std::atoi(e) != 0;
+            if (h->tune.list >= 0) h->use_list = h->nfluid > 0 && h->tune.list != 0;
         }
     }
     h->dirty = false;
@@ -841,7 +845,7 @@ int prepare(lbm* h) {
     const bool ext_force = c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0));
     h->compact_on = h->use_list && !ext_force && h->nfluid <= h->N / 4 && (long long)h->nfluid + h->nbsolid <= h->N &&
                     (long long)h->nfluid + h->nbsolid < (1LL << 28);   // 28-bit extended indices in the neighbour table
-    if (const char* e = std::getenv("LBM_TUNE_COMPACT")) h->compact_on = h->compact_on && std::atoi(e) != 0;
+    if (h->tune.compact >= 0) h->compact_on = h->compact_on && h->tune.compact != 0;
     if (h->compact_on && (unsigned long long)h->q * (((unsigned long long)h->nfluid + 63) / 64 * 64) >= (1ULL << 32))
         h->compact_on = false;   // 32-bit element offsets within a component
     if (h->compact_on) {
@@ -857,7 +861,7 @@ int prepare(lbm* h) {
         int rc = do_launch(h, OP_BUILD_NBR, cmap, nullptr, h->ws + h->cv.nbr);
         if (rc) return rc;
         h->snbr_stride = 0;
-        if (h->nbsolid > 0 && h->nbsolid <= h->N / 4 && !std::getenv("LBM_TUNE_NO_SNBR")) {
+        if (h->nbsolid > 0 && h->nbsolid <= h->N / 4 && !h->tune.no_snbr) {
             h->snbr_stride = ((long long)h->nbsolid + 63) / 64 * 64;
             if ((rc = do_launch(h, OP_BUILD_SNBR, cmap, nullptr, h->ws + h->cv.snbr))) return rc;
         }
@@ -977,15 +981,12 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
         if (cfg->nx % v == 0) h->vec = v;
     }
     h->params_valid = false;
-    h->fvariant = 0;
-    if (const char* e = std::getenv("LBM_TUNE_FUSED_VARIANT")) h->fvariant = std::atoi(e);
-    h->fshape = fused_shape_of(*cfg, h->fvariant);
-    if (h->fshape.vec == 0 && h->fvariant != 0) { h->fvariant = 0; h->fshape = fused_shape_of(*cfg, 0); }
+    h->tune = Tune::from_env();
+    h->fshape = fused_shape_of(*cfg);
     h->fmchunk = 1;
     h->use_fused = false;
     h->feq = false;
     h->eq_half = false;
-    if (const char* e = std::getenv("LBM_TUNE_EQ_HALF")) h->eq_half = std::atoi(e) != 0;
     h->last_path = LBM_PATH_NONE;
     h->gexec = nullptr;
     h->gcur = 0;
@@ -1064,6 +1065,9 @@ int lbm_set_face_bc(lbm_t* h, int face, int kind, const double* rho_w, const dou
     if (h->cfg.periodic[face / 2]) return fail(h, LBM_E_INVALID, "face belongs to a periodic axis");
     if (kind != LBM_FACE_WALL && kind != LBM_FACE_VELOCITY && kind != LBM_FACE_PRESSURE)
         return fail(h, LBM_E_INVALID, "face kind");
+    // the stored planes already hold the face rule of the step before (it is applied at the writing cell): a change
+    // between steps would take effect one step late, so it is only accepted before the first step
+    if (h->initialized && h->steps > 0) return fail(h, LBM_E_STATE, "lbm_set_face_bc after lbm_step: call lbm_init_fields first");
     h->face_kind[face] = kind;
     for (int k = 0; k < 2; ++k) h->face_rho[face][k] = rho_w ? rho_w[k] : 1.0;
     for (int a = 0; a < 3; ++a) h->face_u[face][a] = u_w ? u_w[a] : 0.0;
@@ -1144,8 +1148,8 @@ int lbm_step(lbm_t* h, int n) {
     // ... and each kernel is launched as a programmatic dependent of the one before it (pdl_begin), which hides most of
     // the launch latency between them
     struct PdlScope { lbm* h; ~PdlScope() { h->pdl = false; } } pdl_scope{h};
-    h->pdl = small && !h->profiling && !std::getenv("LBM_TUNE_NO_PDL");
-    if (small && !h->profiling && !h->gfailed && n >= 2 * GRAPH_STEPS + 1 && !std::getenv("LBM_TUNE_NO_GRAPH")) {
+    h->pdl = small && !h->profiling && !h->tune.no_pdl;
+    if (small && !h->profiling && !h->gfailed && n >= 2 * GRAPH_STEPS + 1 && !h->tune.no_graph) {
         if ((rc = step_once())) return rc;      // first step plainly: one-time kernel attribute set-up happens outside capture
         --n;
         if (!h->gvalid) {
@@ -1370,7 +1374,7 @@ int64_t lbm_get_boundary_solids(lbm_t* h, int64_t* out, int64_t capacity) {
                                     h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "boundary solid readback");
-    std::sort(tmp.begin(), tmp.end());
+    std::sort(tmp.begin(), tmp.end());   // the device list is in the brick order of the fluid list
     for (int64_t b = 0; b < h->nbsolid && b < capacity; ++b) out[b] = tmp[(size_t)b];
     return h->nbsolid;
 }

@@ -276,12 +276,12 @@ __device__ __forceinline__ void pull(const KParams<CT>& p, const Cell& c, uint32
 // ------------------------------------------------------------------ pseudopotential (S3)
 // Division and root of the EOS evaluation.  fp32: the hardware approximations (<= 2 ulp) -- the evaluation sits on the
 // critical path of the one-pass kernel's producers, and IEEE division / root cost ~10 instructions each; fp64: exact.
+__device__ __forceinline__ double eos_div(double a, double b) { return a / b; }
 #ifdef LBM_EXACT_EOS
 __device__ __forceinline__ float eos_div(float a, float b) { return a / b; }
 __device__ __forceinline__ float eos_sqrt(float x) { return sqrtf(x); }
 #else
 __device__ __forceinline__ float eos_div(float a, float b) { return __fdividef(a, b); }
-__device__ __forceinline__ double eos_div(double a, double b) { return a / b; }
 __device__ __forceinline__ float eos_sqrt(float x) {
     float r;
     asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));

@@ -3,11 +3,11 @@
 //   k_fused_ws   S1 (rho, j) + S3 (psi) + S4..S7 in ONE pass over the populations
 //                Eq. 4/10, Eq. 12, Eq. 13, Eq. 3, Eq. 5, Eq. 2
 //
-// Same idea as k_fused_v (lbm_fused.cuh): a CTA owns an x-y tile of TX x TY cells, marches along z, and recomputes
-// rho -> psi of the one-cell ring around the tile from the populations, so that the populations cross HBM once per
-// step (B1 = 2 q s bytes per cell instead of B2 = 3 q s + 2 c).  The lock-step version is bound by
-// instruction issue and by its phases (load, barrier, collide) not overlapping.  Here the two halves of the step
-// run concurrently on different planes:
+// A CTA owns an x-y tile of TX x TY cells, marches along z, and recomputes rho -> psi of the one-cell ring around the
+// tile from the populations, so that the populations cross HBM once per step (B1 = 2 q s bytes per cell instead of
+// B2 = 3 q s + 2 c).  (A first, lock-step version -- every warp loads a plane-row into registers, barrier,
+// collide -- was bound by instruction issue and by its phases not overlapping: 5.8 ms on 512^3; removed in round 2.)  Here
+// the two halves of the step run concurrently on different planes:
 //
 //   producers (one warp per tile row incl. the two halo rows, VEC cells per lane, + two warps for the ring columns)
 //       plane p: copy the row segments the pull needs (S7 read side: 19 source rows, one per direction, each with one
@@ -31,17 +31,6 @@
 #include "lbm_hot.cuh"
 
 namespace lbmk {
-
-// Development aid (-DLBM_WS_TIMING): per-role cycle counters accumulated into the (otherwise unused) rho field.
-#ifdef LBM_WS_TIMING
-#define WS_T0() long long t_prev_ = clock64(); long long t_acc_[6] = {0, 0, 0, 0, 0, 0}
-#define WS_TICK(slot) do { const long long t_now_ = clock64(); t_acc_[slot] += t_now_ - t_prev_; t_prev_ = t_now_; } while (0)
-#define WS_FLUSH(base) do { if (lane == 0) { for (int q_ = 0; q_ < 6; ++q_) atomicAdd(reinterpret_cast<unsigned long long*>(p.rho) + (base) + q_, (unsigned long long)t_acc_[q_]); } } while (0)
-#else
-#define WS_T0() do {} while (0)
-#define WS_TICK(slot) do {} while (0)
-#define WS_FLUSH(base) do {} while (0)
-#endif
 
 // ------------------------------------------------------------------ mbarrier / register-split primitives (PTX)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -156,9 +145,9 @@ __device__ __forceinline__ void pulled_from_row(const ST* row, CT (&f)[VEC]) {
     }
 }
 
-template <class L, int NC, class CT, class ST, int COLL, int VEC, int TY, int NSTG, bool WREF, bool PF>
+template <class L, int NC, class CT, class ST, int COLL, int VEC, int TY, int NSTG, bool WREF>
 __global__ void __launch_bounds__((WsTile<L, NC, CT, ST, VEC, TY, NSTG>::THREADS), 1)
-k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
+k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk) {
     using T = WsTile<L, NC, CT, ST, VEC, TY, NSTG>;
     constexpr int Q = L::Q;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -237,11 +226,9 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
         const bool act = cw < nint && xl < txw;
         const int yw = wrap_y(yb + cw);
         const unsigned cell0 = (unsigned)yw * sy + (unsigned)(tx0 + xl);
-        WS_T0();
         for (int m = m0; m < m1; ++m) {
             const int it = m - m0, s = it % NSTG;
             mbar_wait(bar_full + s, (it / NSTG) & 1);
-            WS_TICK(0);
             CT A[NC][Q][VEC];
             if (act) {
                 const ST* rows = stage + (size_t)s * T::STAGE_ELEMS + (size_t)cw * T::ROW_ELEMS + xl;
@@ -257,32 +244,9 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty + s);
-            WS_TICK(1);
-            if constexpr (PF) {
-                // optional L2 prefetch of plane m + pfd of this row (the edge consumers also the halo rows)
-                const int mp = m + pfd;
-                if (pfd > 0 && mp <= m1 && xl < txw && cw < nint) {
-                    const unsigned zq[3] = {(unsigned)wrap_m(mp - 1) * sz, (unsigned)wrap_m(mp) * sz, (unsigned)wrap_m(mp + 1) * sz};
-                    const ST* bC = static_cast<const ST*>(p.f_in) + (tx0 + xl);
-                    auto pf_row = [&](int y) {
-                        const unsigned yq[3] = {(unsigned)wrap_y(y - 1) * sy, (unsigned)y * sy, (unsigned)wrap_y(y + 1) * sy};
-#pragma unroll
-                        for (int k = 0; k < NC; ++k)
-                            static_for<0, Q>([&](auto I) {
-                                constexpr int i = I;
-                                const unsigned idx = (unsigned)(k * Q + i) * plane + zq[1 - L::E[i][2]] + yq[1 - L::E[i][1]];
-                                asm volatile("prefetch.global.L2 [%0];" ::"l"(at_u32(bC, idx)));
-                            });
-                    };
-                    pf_row(yw);
-                    if (cw == 0) pf_row(wrap_y(yb - 1));
-                    if (cw == nint - 1) pf_row(wrap_y(yb + nint));
-                }
-            }
             // psi of planes m-1, m, m+1: plane q (counted from m0-1) lives in slot q % NS
             const int qn = it + 2;
             mbar_wait(bar_psi + (qn % T::NS), (qn / T::NS) & 1);
-            WS_TICK(2);
             if (!act) continue;
             const int sc = (it + 1) % T::NS;
             CT S[NC][3][VEC], pc[NC][VEC];
@@ -331,16 +295,13 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                         else A[k][I][v] = fc[k][I];
                     });
             }
-            WS_TICK(3);
             ST* po = at_u32(static_cast<ST*>(p.f_out), (unsigned)wrap_m(m) * sz + cell0);
 #pragma unroll
             for (int k = 0; k < NC; ++k)
                 static_for<0, Q>([&](auto I) {
                     st_vec_global<CT, ST, VEC>(po + (size_t)(k * Q + I) * plane, A[k][I]);
                 });
-            WS_TICK(4);
         }
-        WS_FLUSH(0);
     };
     // =============================================================== producers
     auto producer_role = [&](int r) {
@@ -397,7 +358,6 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                     }
                 }
             };
-            WS_T0();
             // With more than two stages the copies run AHEAD planes in front of the plane being summed, so that the
             // memory system always has a plane in flight.  (With two stages that does not work: the slot of plane pl+1 is
             // only released once the consumers have collided plane pl-2, and the producer would block in front of a rho
@@ -410,11 +370,9 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                 const bool staged = it >= 0 && pl < m1;       // planes m0-1 and m1 only feed psi
                 const int s = (it + NSTG) % NSTG;
                 if (pl + T::AHEAD <= m1) issue(pl + T::AHEAD);
-                WS_TICK(0);
                 const int q = it + 1, slot = q % T::NS;
                 const ST* land = landing(it);
                 if (used) mbar_wait(bar_land + s * T::ROWS + r, ((it + 1) / NSTG) & 1);
-                WS_TICK(1);
                 if (act) {
 #pragma unroll
                     for (int k = 0; k < NC; ++k) {
@@ -442,15 +400,12 @@ k_fused_ws(const __grid_constant__ KParams<CT> p, int mchunk, int pfd) {
                         st_vec<CT, CT, VEC>(psi_row(slot, k, r) + T::PAD + xl, ps);
                     }
                 }
-                WS_TICK(2);
                 __syncwarp();
                 if (lane == 0) {
                     mbar_arrive(bar_psi + slot);
                     if (staged && r >= 1 && r <= TY) mbar_arrive(bar_full + s);
                 }
-                WS_TICK(3);
             }
-            WS_FLUSH(8);
         }
     };
 

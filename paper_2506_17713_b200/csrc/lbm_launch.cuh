@@ -3,7 +3,6 @@
 #pragma once
 #include <cstdio>
 #include <cstdlib>
-#include "lbm_fused.cuh"
 #include "lbm_fused_ws.cuh"
 #include "lbm_fused_eq.cuh"
 #include "lbm_compact.cuh"
@@ -29,39 +28,23 @@ struct LaunchArgs {
     const void* a1;
     void* a2;
     int i0;              // op-specific integer (OP_FUSED: planes marched per CTA)
-    int variant;         // OP_FUSED: 0 = default (warp-specialised k_fused_ws on D3Q19, lock-step k_fused_v on D2Q9);
-                         //           -1 = lock-step kernel everywhere; 1.. = tuning experiments (LBM_FUSED_TUNING)
-    int pfd;             // OP_FUSED (warp-specialised): L2 prefetch distance in planes
     int eq;              // OP_FUSED: one component, BGK, tau = 1 (f* is an equilibrium): the row-pipeline kernel k_fused_eq applies
+                         //           (2: with half-width tiles and two CTAs per SM)
     int* used_kernel;    // OP_FUSED, out: the lbm_path value of the kernel that ran
     int wref;            // OP_FUSED: rho_ref != 0 (populations stored shifted by w_i rho_ref)
     int pdl;             // OP_MOMENTS / OP_VIRTUAL / OP_STEP (dense mapping): programmatic dependent launch (pdl_begin)
     cudaStream_t stream;
 };
 
-// Tile of the one-pass kernel K2F per (lattice, dtypes, components): VEC cells per lane, WX warps per row, TY rows.
+// Tile of the one-pass kernels K2F (D3Q19) per (dtypes, components): VEC cells per lane (tile width 32 x VEC), TY rows.
 // VEC = 0: no one-pass kernel built for this combination (the two-pass path is used).
-struct FusedShape { int vec, wx, ty; };
+struct FusedShape { int vec, ty; };
 template <class L, class CT, class ST, int NC>
 constexpr FusedShape fused_shape() {
-    constexpr bool d3 = L::D == 3;
-    if (sizeof(CT) == 4) return NC == 1 ? FusedShape{4, 1, d3 ? 8 : 1} : FusedShape{2, 1, d3 ? 8 : 1};
-    return NC == 1 ? FusedShape{2, 1, d3 ? 8 : 1} : FusedShape{0, 0, 0};
+    if (L::D != 3) return FusedShape{0, 0};
+    if (sizeof(CT) == 4) return NC == 1 ? FusedShape{4, 8} : FusedShape{2, 8};
+    return NC == 1 ? FusedShape{2, 8} : FusedShape{0, 0};
 }
-// Tuning experiments of K2F (built with -DLBM_FUSED_TUNING; D3Q19, fp32 compute, one component, BGK only):
-// variant v = 1..FUSED_TUNING_VARIANTS selects {shape, L2 prefetch}; 0 is the default shape above.
-constexpr int FUSED_TUNING_VARIANTS = 6;
-constexpr FusedShape fused_tuning_shape(int v) {
-    switch (v) {
-        case 1: return {4, 1, 8};
-        case 2: return {2, 1, 14};
-        case 3: return {2, 1, 14};
-        case 4: return {2, 2, 6};
-        case 5: return {4, 1, 6};
-        default: return {2, 1, 8};
-    }
-}
-constexpr bool fused_tuning_pf(int v) { return v != 1 && v != 3; }
 
 template <class L, class CT, class ST>
 cudaError_t launch(const LaunchArgs& a);
@@ -227,111 +210,67 @@ cudaError_t launch(const LaunchArgs& a) {
         }
         case OP_FUSED: {
             bool done = false;
+            int dev = 0;
+            cudaGetDevice(&dev);
+            // dynamic shared memory opt-in and the register pool the kernels re-split with setmaxnreg (a smaller pool would make
+            // setmaxnreg.inc wait forever): checked once per device and kernel
+            auto usable = [&](auto kern, int (&ready)[16], size_t smem, long long regs_needed, int threads) {
+                int& rd = ready[dev & 15];   // 0 unknown, 1 usable, -1 not usable
+                if (rd == 0) {
+                    cudaFuncAttributes fa;
+                    const cudaError_t e1 = cudaFuncGetAttributes(&fa, kern);
+                    const bool regs_ok = e1 == cudaSuccess && (long long)fa.numRegs * threads >= regs_needed;
+                    const cudaError_t e2 = regs_ok ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                                                   : cudaErrorUnknown;
+                    rd = (regs_ok && e2 == cudaSuccess) ? 1 : -1;
+                    cudaGetLastError();
+                }
+                return rd > 0;
+            };
             with_nc([&](auto NC) {
                 auto with_coll = [&](auto fn) {
                     if (a.coll == 0) fn(IC<0>{});
                     else if (a.coll == 1) fn(IC<1>{});
                 };
                 with_coll([&](auto C_) {
-                    auto go = [&](auto VEC, auto WX, auto TY, auto PF) {
-                        using T = FusedTile<L, NC, CT, VEC, WX, TY>;
-                        dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), 1, 1);
-                        if (L::D == 3) {
-                            g.y = (unsigned)((p.ny + TY - 1) / TY);
-                            g.z = (unsigned)((p.nz + a.i0 - 1) / a.i0);
-                        } else {
-                            g.y = (unsigned)((p.ny + a.i0 - 1) / a.i0);
-                        }
-                        k_fused_v<L, NC, CT, ST, C_, VEC, WX, TY, (PF != 0)><<<g, T::THREADS, 0, a.stream>>>(p, a.i0);
-                        if (a.used_kernel) *a.used_kernel = 2;  // LBM_PATH_ONE_PASS_LOCKSTEP
-                        done = true;
-                    };
                     constexpr FusedShape fs = fused_shape<L, CT, ST, NC>();
-                    // warp-specialised pipeline (D3Q19): needs the dynamic shared memory opt-in and the register pool
-                    // it re-splits with setmaxnreg (a smaller pool would make setmaxnreg.inc wait forever)
-                    auto go_ws = [&](auto VEC, auto TY, auto NSTG, auto WREF, auto PF) {
-                        if constexpr (L::D == 3) {
-                            using T = WsTile<L, NC, CT, ST, VEC, TY, NSTG>;
-                            auto kern = k_fused_ws<L, NC, CT, ST, C_, VEC, TY, NSTG, (WREF != 0), (PF != 0)>;
-                            static int ready = 0;   // 0 unknown, 1 usable, -1 not usable
-                            if (ready == 0) {
-                                cudaFuncAttributes fa;
-                                const cudaError_t e1 = cudaFuncGetAttributes(&fa, kern);
-                                const bool regs_ok = e1 == cudaSuccess &&
-                                                     fa.numRegs * T::THREADS >= T::REG_PROD * T::NPW * 32 + T::REG_CONS * T::NCW * 32;
-                                const cudaError_t e2 = regs_ok ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                                                      (int)T::SMEM) : cudaErrorUnknown;
-                                ready = (regs_ok && e2 == cudaSuccess) ? 1 : -1;
-                                if (ready < 0 && std::getenv("LBM_VERBOSE"))
-                                    std::fprintf(stderr, "[lbm] k_fused_ws unusable: attr=%s regs=%d smem=%zu set=%s; lock-step kernel used\n",
-                                                 cudaGetErrorString(e1), e1 == cudaSuccess ? fa.numRegs : -1, (size_t)T::SMEM,
-                                                 cudaGetErrorString(e2));
-                                cudaGetLastError();
-                            }
-                            if (ready < 0) return;
-                            dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + TY - 1) / TY),
-                                   (unsigned)((p.nz + a.i0 - 1) / a.i0));
-                            kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0, a.pfd);
-                            if (a.used_kernel) *a.used_kernel = 3;  // LBM_PATH_ONE_PASS_WS
-                            done = true;
-                        }
-                    };
-                    // row-pipeline kernel (lbm_fused_eq.cuh): same tile, same opt-ins
-                    auto go_eq = [&](auto VEC, auto TY, auto CPS, auto WREF) {
-                        if constexpr (L::D == 3 && NC == 1 && C_ == 0) {
-                            using T = EqTile<L, CT, ST, VEC, TY, CPS>;
-                            auto kern = k_fused_eq<L, CT, ST, VEC, TY, CPS, (WREF != 0)>;
-                            static int ready[16] = {0};   // per device: 0 unknown, 1 usable, -1 not usable
-                            int dev = 0;
-                            cudaGetDevice(&dev);
-                            int& rd = ready[dev & 15];
-                            if (rd == 0) {
-                                cudaFuncAttributes fa;
-                                const cudaError_t e1 = cudaFuncGetAttributes(&fa, kern);
-                                // the register pool the kernel re-splits with setmaxnreg (a smaller one would make setmaxnreg.inc wait forever)
-                                const bool regs_ok = e1 == cudaSuccess &&
-                                                     fa.numRegs * T::THREADS >= T::REG_PROD * T::NPW * 32 + T::REG_CONS * T::NCW * 32;
-                                const cudaError_t e2 = regs_ok ? cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                                                      (int)T::SMEM) : cudaErrorUnknown;
-                                rd = (regs_ok && e2 == cudaSuccess) ? 1 : -1;
-                                cudaGetLastError();
-                            }
-                            if (rd < 0) return;
-                            dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + TY - 1) / TY),
+                    if constexpr (fs.vec > 0) {
+                        // k_fused_ws: warp-specialised producer / consumer pipeline, two stages of fs.ty rows
+                        auto go_ws = [&](auto WREF) {
+                            using T = WsTile<L, NC, CT, ST, fs.vec, fs.ty, 2>;
+                            auto kern = k_fused_ws<L, NC, CT, ST, C_, fs.vec, fs.ty, 2, (WREF != 0)>;
+                            static int ready[16] = {0};
+                            if (!usable(kern, ready, T::SMEM, (long long)T::REG_PROD * T::NPW * 32 + (long long)T::REG_CONS * T::NCW * 32, T::THREADS)) return;
+                            dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + fs.ty - 1) / fs.ty),
                                    (unsigned)((p.nz + a.i0 - 1) / a.i0));
                             kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0);
-                            if (a.used_kernel) *a.used_kernel = 5;  // LBM_PATH_ONE_PASS_EQ
+                            if (a.used_kernel) *a.used_kernel = 3;  // LBM_PATH_ONE_PASS_WS
                             done = true;
+                        };
+                        // k_fused_eq: row pipelines (lbm_fused_eq.cuh); CPS = 2: half-width tiles, two CTAs per SM
+                        auto go_eq = [&](auto VEC, auto CPS, auto WREF) {
+                            if constexpr (NC == 1 && C_ == 0) {
+                                using T = EqTile<L, CT, ST, VEC, fs.ty, CPS>;
+                                auto kern = k_fused_eq<L, CT, ST, VEC, fs.ty, CPS, (WREF != 0)>;
+                                static int ready[16] = {0};
+                                if (!usable(kern, ready, T::SMEM, (long long)T::REG_PROD * T::NPW * 32 + (long long)T::REG_CONS * T::NCW * 32, T::THREADS)) return;
+                                dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + fs.ty - 1) / fs.ty),
+                                       (unsigned)((p.nz + a.i0 - 1) / a.i0));
+                                kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0);
+                                if (a.used_kernel) *a.used_kernel = 5;  // LBM_PATH_ONE_PASS_EQ
+                                done = true;
+                            }
+                        };
+                        if (a.eq == 2) {
+                            if (a.wref) go_eq(IC<fs.vec / 2>{}, IC<2>{}, IC<1>{});
+                            else go_eq(IC<fs.vec / 2>{}, IC<2>{}, IC<0>{});
+                        } else if (a.eq == 1) {
+                            if (a.wref) go_eq(IC<fs.vec>{}, IC<1>{}, IC<1>{});
+                            else go_eq(IC<fs.vec>{}, IC<1>{}, IC<0>{});
                         }
-                    };
-                    if constexpr (fs.vec > 0) {
-                        if constexpr (L::D == 3) {
-                            if (a.variant == 0 && a.eq) {
-                                if (a.eq == 2) {       // half-width tiles, two CTAs per SM
-                                    if (a.wref) go_eq(IC<fs.vec / 2>{}, IC<fs.ty>{}, IC<2>{}, IC<1>{});
-                                    else go_eq(IC<fs.vec / 2>{}, IC<fs.ty>{}, IC<2>{}, IC<0>{});
-                                } else {
-                                    if (a.wref) go_eq(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{}, IC<1>{});
-                                    else go_eq(IC<fs.vec>{}, IC<fs.ty>{}, IC<1>{}, IC<0>{});
-                                }
-                                if (done) return;
-                            }
-                            // default: two stages of 8 rows.  Variant 12 = three stages of 6 rows (one component only: it
-                            // decouples producers and consumers further but the smaller tile re-reads more; measured slower)
-                            if (a.variant == 0) {
-                                if (a.wref) go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<2>{}, IC<1>{}, IC<1>{});
-                                else go_ws(IC<fs.vec>{}, IC<fs.ty>{}, IC<2>{}, IC<0>{}, IC<1>{});
-                                if (done) return;
-                            }
-                            // variant 13: half-width tiles (VEC / 2) and four stages, the copies two planes ahead
-                            if constexpr (NC == 1 && sizeof(CT) == 4) {
-                                if (a.variant == 13 && !a.wref) {
-                                    go_ws(IC<fs.vec / 2>{}, IC<8>{}, IC<4>{}, IC<0>{}, IC<1>{});
-                                    if (done) return;
-                                }
-                            }
-                        }
-                        go(IC<fs.vec>{}, IC<fs.wx>{}, IC<fs.ty>{}, IC<1>{});
+                        if (done) return;
+                        if (a.wref) go_ws(IC<1>{});
+                        else go_ws(IC<0>{});
                     }
                 });
             });

@@ -1,9 +1,9 @@
-"""GPU parity of the one-pass kernel K2F (lbm_fused.cuh) against the oracle and against the two-pass path.
+"""GPU parity of the one-pass kernels K2F (k_fused_ws, k_fused_eq; D3Q19) against the oracle and against the two-pass path.
 
 K2F recomputes rho -> psi of the ring around its tile instead of reading a psi field written by K1, so the
 cases here stress what is new: tiles with ragged edges in x and y, several marching chunks, wrap-around of
-the ring columns and rows, domains smaller than one tile, both lattices, all dtype combinations it is built
-for, two components, MRT and both forcing schemes.  Gates are those of test_gpu_parity.py.
+the ring columns and rows, domains smaller than one tile, all dtype combinations it is built for, two
+components, MRT and both forcing schemes.  Gates are those of test_gpu_parity.py.
 """
 import numpy as np
 import pytest
@@ -31,25 +31,24 @@ def run_three(wl, inp, steps, oracle_wl=None):
     g1.step(steps)
     assert g1.kernel_launches - l0 == steps      # one launch per step: K2F ran, not K1 + K2
     import os
-    # k_fused_ws: D3Q19 and rows that are whole 16-byte vectors of the storage dtype; else the lock-step kernel
-    sbytes = {"f16": 2, "f32": 4, "f64": 8}[wl.get("store_dtype", wl.get("compute_dtype", "f64"))]
-    ws = wl["lattice"] == "D3Q19" and wl["nx"] % (16 // sbytes) == 0 and os.environ.get("LBM_TUNE_FUSED_VARIANT") != "-1"
-    # ... and the row-pipeline kernel k_fused_eq where the collision result is an equilibrium (one component, BGK, tau = 1)
-    eq = ws and wl["n_components"] == 1 and wl.get("collision", "BGK") == "BGK" and list(wl.get("tau", [1.0])) == [1.0] \
+    # k_fused_eq where the collision result is an equilibrium (one component, BGK, tau = 1), else k_fused_ws
+    eq = wl["n_components"] == 1 and wl.get("collision", "BGK") == "BGK" and list(wl.get("tau", [1.0])) == [1.0] \
         and not os.environ.get("LBM_TUNE_NO_EQ")
-    want = "one_pass_eq" if eq else "one_pass_ws" if ws else "one_pass_lockstep"
+    want = "one_pass_eq" if eq else "one_pass_ws"
     assert g1.hot_path == want, g1.hot_path        # and the intended kernel, not a silent fallback
     g2.step(steps)
     return ([o.get_populations(k) for k in range(o.nc)], [g1.get_populations(k) for k in range(o.nc)],
             [g2.get_populations(k) for k in range(o.nc)], o)
 
 
-@pytest.mark.parametrize("kernel", ["warp_specialised", "lock_step"])
+@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_ws"])
 @pytest.mark.parametrize("dims", [(128, 24, 20), (132, 9, 11), (4, 3, 2), (260, 8, 5), (8, 35, 3)])
 def test_d3q19_fp64_ragged_tiles(dims, kernel, monkeypatch):
     monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "7")   # several marching chunks, ragged last one
-    if kernel == "lock_step":                           # k_fused_v instead of k_fused_ws (lbm_launch.cuh)
-        monkeypatch.setenv("LBM_TUNE_FUSED_VARIANT", "-1")
+    if kernel == "k_fused_ws":                          # the general kernel where k_fused_eq would apply
+        monkeypatch.setenv("LBM_TUNE_NO_EQ", "1")
+    else:
+        monkeypatch.setenv("LBM_TUNE_EQ_HALF", "1" if kernel == "k_fused_eq_half" else "0")
     wl, _ = W.config5(16, "f64")
     wl.update(nx=dims[0], ny=dims[1], nz=dims[2])
     inp = small_inputs(wl, 21, 0.05, 0.3)
@@ -59,10 +58,12 @@ def test_d3q19_fp64_ragged_tiles(dims, kernel, monkeypatch):
     assert_parity(f2, f1, fluid, 1e-13, relative=False)   # same arithmetic in the same order as K2
 
 
-@pytest.mark.parametrize("kernel", ["warp_specialised", "lock_step"])
+@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_ws"])
 def test_config5_fp32_100_steps(kernel, monkeypatch):
-    if kernel == "lock_step":
-        monkeypatch.setenv("LBM_TUNE_FUSED_VARIANT", "-1")
+    if kernel == "k_fused_ws":
+        monkeypatch.setenv("LBM_TUNE_NO_EQ", "1")
+    else:
+        monkeypatch.setenv("LBM_TUNE_EQ_HALF", "1" if kernel == "k_fused_eq_half" else "0")
     wl, inp = W.config5(48, "f32")
     fo, f1, f2, o = run_three(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
     fluid = np.ones(o.N, bool)
@@ -118,17 +119,7 @@ def test_config3_mrt_peng_robinson_fp64():
     assert_parity(fo, f1, np.ones(o.N, bool), TOL64, relative=False)
 
 
-@pytest.mark.parametrize("nx,ny", [(64, 64), (70, 37), (200, 3), (2, 5)])
-def test_d2q9_fp64(nx, ny, monkeypatch):
-    monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "9")
-    wl, _ = W.config1(8, "f64")
-    wl.update(nx=nx, ny=ny)
-    inp = small_inputs(wl, 11, 0.05, 0.25)
-    fo, f1, f2, o = run_three(wl, inp, 100)
-    assert_parity(fo, f1, np.ones(o.N, bool), TOL64, relative=False)
-
-
-@pytest.mark.parametrize("lattice,n", [("D2Q9", (46, 23, 1)), ("D3Q19", (24, 10, 9)), ("D3Q19", (22, 10, 9))])
+@pytest.mark.parametrize("lattice,n", [("D3Q19", (24, 10, 9)), ("D3Q19", (136, 19, 6))])
 @pytest.mark.parametrize("collision", ["BGK", "MRT"])
 @pytest.mark.parametrize("forcing", ["EDM", "SHIFT"])
 def test_two_components_variants_fp32(lattice, n, collision, forcing):
@@ -150,8 +141,12 @@ def test_one_pass_refused_where_it_does_not_apply():
     with pytest.raises(binding.LBMError):
         s.step(1)
     wl, inp = W.config5(16, "f32")
-    wl.update(nx=18)                                     # nx not a multiple of the vector width
+    wl.update(nx=18)                                     # rows that are not whole 16-byte vectors
     inp = small_inputs(wl, 1)
+    s = make_gpu(one_pass(wl), inp)
+    with pytest.raises(binding.LBMError):
+        s.step(1)
+    wl, inp = W.config1(32, "f64")                       # D2Q9: no one-pass kernel (the two-pass path wins there)
     s = make_gpu(one_pass(wl), inp)
     with pytest.raises(binding.LBMError):
         s.step(1)

@@ -373,6 +373,23 @@ def test_api_state_and_errors():
     assert g.L.lbm_create(C.byref(cfg), C.c_void_p(ws.data_ptr() + 8), need, None, C.byref(h)) == -3
     host = np.zeros(16, dtype=np.uint8)
     assert g.L.lbm_create(C.byref(cfg), host.ctypes.data_as(C.c_void_p), need, None, C.byref(h)) in (-1, -3)
+    # a face rule is folded into the stored populations at the writing cell: it cannot change once steps have run
+    wlc, inpc = W.config4(24, store_dtype="f32")
+    gc = make_gpu(wlc, inpc)
+    gc.set_face_bc(0, "VELOCITY", (1.0, 0.03), (2e-3, 0.0, 0.0))        # between init and the first step: accepted
+    oc = make_oracle(with_dtype(wlc, "f64"), inpc)
+    oc.set_face_bc(0, "VELOCITY", (1.0, 0.03), (2e-3, 0.0, 0.0))
+    gc.step(5); oc.step(5)
+    fl = fluid_mask(inpc, oc.N)
+    assert_parity([oc.get_populations(k) for k in range(2)], [gc.get_populations(k) for k in range(2)], fl, TOL32, relative=True)
+    with pytest.raises(binding.LBMError, match="LBM_E_STATE"):
+        gc.set_face_bc(0, "VELOCITY", (1.0, 0.03), (1e-3, 0.0, 0.0))
+    # MRT rate sets whose momentum rows differ are rejected (include/lbm.h: mrt_rates)
+    wlm, _ = W.config3(16, "f64")
+    rates = list(W.mrt_rates("D3Q19", 1.0))
+    rates[5] = 1.1
+    with pytest.raises(binding.LBMError):
+        binding.LBM(dict(wlm, mrt_rates=[rates]))
 
 
 def test_device_resident_io_and_reinit():
