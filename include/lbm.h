@@ -248,7 +248,8 @@ enum lbm_path {
     LBM_PATH_RESERVED_2 = 2,        /* (round 1's lock-step one-pass kernel; removed) */
     LBM_PATH_ONE_PASS_WS = 3,       /* K2F k_fused_ws (warp-specialised, bulk asynchronous copies) */
     LBM_PATH_TWO_PASS_COMPACT = 4,  /* K1 (+K1b) + K2 on the fluid-compact layout (at most a quarter of the cells fluid) */
-    LBM_PATH_ONE_PASS_EQ = 5        /* K2F k_fused_eq (row pipelines; one component, BGK with tau = 1) */
+    LBM_PATH_ONE_PASS_EQ = 5,       /* K2F k_fused_eq (row pipelines; one component, BGK with tau = 1) */
+    LBM_PATH_TWO_PASS_PERSISTENT = 6 /* K1 | K1b | K2 as phases of one persistent cooperative kernel (small domains, n >= 2) */
 };
 LBM_API int lbm_hot_path(const lbm_t* h);
 

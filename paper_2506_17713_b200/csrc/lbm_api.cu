@@ -83,6 +83,7 @@ struct lbm {
     int gcur;            // buffer parity the graph was captured at
     int64_t glaunches;   // kernels per replay
     bool gvalid, gfailed;
+    bool coop_failed;    // the cooperative launch of the persistent small-domain kernel is not available
     bool initialized, has_solid, bnd, dirty, force_rho;
     int nbsolid;
     int nfluid;       // fluid cells (masked domains)
@@ -993,6 +994,7 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->glaunches = 0;
     h->gvalid = false;
     h->gfailed = false;
+    h->coop_failed = false;
     h->initialized = false;
     h->has_solid = false;
     h->dirty = true;
@@ -1140,13 +1142,29 @@ int lbm_step(lbm_t* h, int n) {
         h->steps++;
         return LBM_OK;
     };
-    // Small domains are bound by kernel launches (a D2Q9 64 x 64 step is two ~3 us kernels): GRAPH_STEPS steps are
-    // captured once into a CUDA graph and replayed.  Not while profiling (event brackets), not on a stream that cannot
+    // Small domains are bound by kernel launches (a D2Q9 64 x 64 step is two ~3 us kernels).  First choice: ONE persistent
+    // kernel for all n steps (lbm_small.cuh: resident CTAs, grid barriers between the phases).  Where the cooperative launch
+    // is not available: GRAPH_STEPS steps are captured once into a CUDA graph and replayed.  Not while profiling (event brackets), not on a stream that cannot
     // be captured (the legacy default stream): then, and for large domains, the kernels are launched one by one.
     constexpr int GRAPH_STEPS = 16;   // even: the ping-pong parity is the same after a replay
     const bool small = (long long)h->N * h->cfg.n_components <= (1LL << 22);
     // ... and each kernel is launched as a programmatic dependent of the one before it (pdl_begin), which hides most of
     // the launch latency between them
+    const bool ext_force = h->cfg.zc_A[0] != 0.0 || h->cfg.st_kappa[0] != 0.0 ||
+                           (h->cfg.n_components > 1 && (h->cfg.zc_A[1] != 0.0 || h->cfg.st_kappa[1] != 0.0));
+    if (small && n >= 2 && !h->profiling && !h->coop_failed && !h->tune.no_coop && !h->use_fused && !h->use_list && !ext_force) {
+        unsigned* ctr = reinterpret_cast<unsigned*>(h->ws + h->cv.counter + 64);
+        CU(cudaMemsetAsync(ctr, 0, sizeof(unsigned), h->stream));
+        rc = do_launch(h, OP_COOP, nullptr, nullptr, ctr, n);
+        if (rc == LBM_OK) {
+            h->cur ^= (n & 1);
+            h->steps += n;
+            h->last_path = LBM_PATH_TWO_PASS_PERSISTENT;
+            return LBM_OK;
+        }
+        h->coop_failed = true;   // not available / more cells than resident threads: the graph or plain launches below
+        h->err.clear();
+    }
     struct PdlScope { lbm* h; ~PdlScope() { h->pdl = false; } } pdl_scope{h};
     h->pdl = small && !h->profiling && !h->tune.no_pdl;
     if (small && !h->profiling && !h->gfailed && n >= 2 * GRAPH_STEPS + 1 && !h->tune.no_graph) {
