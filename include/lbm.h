@@ -218,6 +218,28 @@ LBM_API int lbm_get_psi(lbm_t* h, int comp, void* psi, int dtype, int on_device)
 LBM_API int lbm_render_isosurface(lbm_t* h, int comp, double iso, int axis, void* shade, void* depth, int dtype,
                                   int on_device);
 
+/* ---- Slab decomposition along the LAST axis (z for D3Q19, y for D2Q9): the multi-GPU exchange step.
+ * A rank's handle holds its slab of the global domain plus `width` ghost layers below and above it along the last
+ * axis, is configured PERIODIC along that axis (the wrap only ever feeds ghost layers) and steps as usual; before every
+ * lbm_step the ghost layers are overwritten with the neighbours' outermost interior layers:
+ *     lbm_export_halo(side)  packs the `width` interior layers next to the ghost layers of `side` (0: low, 1: high),
+ *     lbm_import_halo(side)  overwrites the `width` ghost layers of `side` with a packed buffer,
+ * so rank r's export(1) is rank r+1's import(0) and rank r+1's export(0) is rank r's import(1).  width = 2 for a plain
+ * Shan-Chen step (the force at the outermost interior layer reads psi one layer out, Eq. 13, and psi there is taken from
+ * populations pulled one layer further, Eq. 2 + Eq. 12), width = 3 when solid cells with virtual density (Eq. 17) can
+ * lie in the ghost layers.  The solid mask passed to lbm_set_solid_mask covers the ghost layers too.  After a step the
+ * ghost layers hold values computed from wrapped data; they are never read by an owned cell before the next import --
+ * by lbm_step, that is: the exports (lbm_get_populations, lbm_get_macroscopic, lbm_render_isosurface) return post-stream
+ * values, which the outermost owned layer pulls from the first ghost layer, so exchange once more before exporting.
+ * Buffer: device memory, lbm_halo_bytes() bytes, [component][direction][layer][cells of a layer] in the STORAGE dtype --
+ * the stored (post-collision, R14) populations, moved as bytes; 16-byte alignment makes the copy vectorised, alignment
+ * to the storage dtype is required.  Asynchronous on the handle's stream; one copy kernel per call.
+ * Errors: LBM_E_INVALID (side, width < 1 or 3 * width > layers, last axis not periodic, alignment), LBM_E_STATE before
+ * lbm_init_fields.  A handle in the fluid-compact layout is converted back to the dense one first. */
+LBM_API int lbm_halo_bytes(lbm_t* h, int width, size_t* bytes);
+LBM_API int lbm_export_halo(lbm_t* h, int side, int width, void* d_buf);
+LBM_API int lbm_import_halo(lbm_t* h, int side, int width, const void* d_buf);
+
 /* Lattice tables: q, e[q][3], w[q], opposite[q].  Host pointers; any may be NULL. */
 LBM_API int lbm_get_lattice(int lattice, int* q, int* e, double* w, int* opposite);
 

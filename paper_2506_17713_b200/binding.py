@@ -77,6 +77,9 @@ _SIGNATURES = {
     "lbm_get_lattice": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "lbm_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
     "lbm_get_kernel_times": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "lbm_halo_bytes": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "lbm_export_halo": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
+    "lbm_import_halo": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "lbm_hot_path": (C.c_int, [C.c_void_p]),
     "lbm_steps_done": (C.c_int64, [C.c_void_p]),
     "lbm_kernel_launches": (C.c_int64, [C.c_void_p]),
@@ -311,6 +314,23 @@ class LBM:
         assert f.shape == (self.q, self.N)
         self._check(self.L.lbm_set_populations(self.h, k, f.ctypes.data_as(C.c_void_p), _np_dtype_code(f), 0),
                     "lbm_set_populations")
+
+    # ---- slab decomposition (include/lbm.h): packed halo layers as uint8 device tensors
+    def halo_bytes(self, width: int) -> int:
+        n = C.c_size_t(0)
+        self._check(self.L.lbm_halo_bytes(self.h, int(width), C.byref(n)), "lbm_halo_bytes")
+        return int(n.value)
+
+    def export_halo(self, side: int, width: int, out=None):
+        if out is None:
+            out = self.torch.empty(self.halo_bytes(width), dtype=self.torch.uint8, device=self.device)
+        assert out.is_cuda and out.is_contiguous() and out.numel() >= self.halo_bytes(width)
+        self._check(self.L.lbm_export_halo(self.h, int(side), int(width), C.c_void_p(out.data_ptr())), "lbm_export_halo")
+        return out
+
+    def import_halo(self, side: int, width: int, buf):
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() >= self.halo_bytes(width)
+        self._check(self.L.lbm_import_halo(self.h, int(side), int(width), C.c_void_p(buf.data_ptr())), "lbm_import_halo")
 
     def get_link_flags(self) -> np.ndarray:
         out = np.empty(self.N, dtype=np.uint32)

@@ -111,6 +111,18 @@ struct lbm {
     int64_t k_cnt[LBM_K_COUNT];
 };
 
+// Halo layers of the slab decomposition (lbm_export_halo / lbm_import_halo): `rows` chunks of `row_units` units of U bytes,
+// chunk r at src + r * src_pitch -> dst + r * dst_pitch (pitches in units).  Pure data movement in the storage dtype.
+template <class U>
+__global__ void __launch_bounds__(256) k_halo_copy(U* __restrict__ dst, const U* __restrict__ src, long long rows, long long row_units,
+                                                   long long src_pitch, long long dst_pitch) {
+    const long long total = rows * row_units;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long r = t / row_units, c = t - r * row_units;
+        dst[r * dst_pitch + c] = src[r * src_pitch + c];
+    }
+}
+
 namespace {
 
 int q_of(int lattice) { return lattice == LBM_D2Q9 ? 9 : 19; }
@@ -936,6 +948,47 @@ int deliver_output(lbm* h, const void* dev, long long n, int dtype, int on_devic
 }  // namespace
 
 // ==================================================================== C ABI
+// ---- slab decomposition along the last axis: halo layers in the storage dtype, [component][direction][layer][cells of a layer]
+namespace {
+struct HaloGeom { long long layer, nl, chunk_bytes, plane_bytes; int rows; };
+int halo_geom(lbm* h, int width, HaloGeom* g) {
+    const lbm_config_t& c = h->cfg;
+    g->layer = h->d == 3 ? (long long)c.nx * c.ny : (long long)c.nx;
+    g->nl = h->d == 3 ? c.nz : c.ny;
+    if (width < 1 || 3LL * width > g->nl) return fail(h, LBM_E_INVALID, "halo width: the last axis needs at least 3 * width layers");
+    if (!c.periodic[h->d - 1]) return fail(h, LBM_E_INVALID, "halo exchange: the handle must be periodic along its last axis");
+    g->chunk_bytes = (long long)width * g->layer * (long long)h->sbytes;
+    g->plane_bytes = h->plane * (long long)h->sbytes;
+    g->rows = c.n_components * h->q;
+    return LBM_OK;
+}
+// copy the layers [l0, l0 + width) of every population plane to / from a packed buffer
+int halo_copy(lbm* h, const HaloGeom& g, long long l0, void* packed, bool to_packed) {
+    char* planes = h->ws + h->cv.f[h->cur] + l0 * g.layer * (long long)h->sbytes;
+    if ((uintptr_t)packed % (uintptr_t)h->sbytes != 0) return fail(h, LBM_E_INVALID, "halo buffer alignment");
+    const bool a16 = g.chunk_bytes % 16 == 0 && g.plane_bytes % 16 == 0 && ((uintptr_t)planes % 16) == 0 && ((uintptr_t)packed % 16) == 0;
+    const long long unit = a16 ? 16 : (long long)h->sbytes;
+    const long long ru = g.chunk_bytes / unit, pp = g.plane_bytes / unit, total = ru * g.rows;
+    const unsigned blocks = (unsigned)std::min<long long>((total + 255) / 256, 148LL * 16);
+    char* dst = to_packed ? static_cast<char*>(packed) : planes;
+    const char* src = to_packed ? planes : static_cast<const char*>(packed);
+    const long long sp = to_packed ? pp : ru, dp = to_packed ? ru : pp;
+    if (unit == 16) k_halo_copy<uint4><<<blocks, 256, 0, h->stream>>>((uint4*)dst, (const uint4*)src, g.rows, ru, sp, dp);
+    else if (unit == 8) k_halo_copy<uint2><<<blocks, 256, 0, h->stream>>>((uint2*)dst, (const uint2*)src, g.rows, ru, sp, dp);
+    else if (unit == 4) k_halo_copy<uint32_t><<<blocks, 256, 0, h->stream>>>((uint32_t*)dst, (const uint32_t*)src, g.rows, ru, sp, dp);
+    else k_halo_copy<uint16_t><<<blocks, 256, 0, h->stream>>>((uint16_t*)dst, (const uint16_t*)src, g.rows, ru, sp, dp);
+    CU(cudaGetLastError());
+    h->launches++;
+    return LBM_OK;
+}
+int halo_ready(lbm* h) {
+    if (!h->initialized) return fail(h, LBM_E_STATE, "halo exchange before lbm_init_fields");
+    int rc = prepare(h);
+    if (rc) return rc;
+    return set_layout(h, false);
+}
+}  // namespace
+
 extern "C" {
 
 size_t lbm_workspace_bytes(const lbm_config_t* cfg) {
@@ -1443,6 +1496,33 @@ int lbm_get_lattice(int lattice, int* q, int* e, double* w, int* opposite_out) {
     if (lattice == LBM_D2Q9) fill(D2Q9{});
     else fill(D3Q19{});
     return LBM_OK;
+}
+
+int lbm_halo_bytes(lbm_t* h, int width, size_t* bytes) {
+    if (!h || !bytes) return LBM_E_INVALID;
+    HaloGeom g;
+    const int rc = halo_geom(h, width, &g);
+    if (rc) return rc;
+    *bytes = (size_t)g.chunk_bytes * (size_t)g.rows;
+    return LBM_OK;
+}
+
+int lbm_export_halo(lbm_t* h, int side, int width, void* d_buf) {
+    if (!h || !d_buf || (side != 0 && side != 1)) return LBM_E_INVALID;
+    HaloGeom g;
+    int rc = halo_geom(h, width, &g);
+    if (rc) return rc;
+    if ((rc = halo_ready(h))) return rc;
+    return halo_copy(h, g, side == 0 ? width : g.nl - 2LL * width, d_buf, true);
+}
+
+int lbm_import_halo(lbm_t* h, int side, int width, const void* d_buf) {
+    if (!h || !d_buf || (side != 0 && side != 1)) return LBM_E_INVALID;
+    HaloGeom g;
+    int rc = halo_geom(h, width, &g);
+    if (rc) return rc;
+    if ((rc = halo_ready(h))) return rc;
+    return halo_copy(h, g, side == 0 ? 0 : g.nl - (long long)width, const_cast<void*>(d_buf), false);
 }
 
 int lbm_hot_path(const lbm_t* h) { return h ? h->last_path : LBM_E_INVALID; }
