@@ -240,6 +240,28 @@ LBM_API int lbm_halo_bytes(lbm_t* h, int width, size_t* bytes);
 LBM_API int lbm_export_halo(lbm_t* h, int side, int width, void* d_buf);
 LBM_API int lbm_import_halo(lbm_t* h, int side, int width, const void* d_buf);
 
+/* ---- One time step without any allocation and without a handle or workspace: for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+ * lbm_step_noalloc runs S1..S7 once, as the two-pass arrangement K1 (rho, psi) -> K2 (force, collision, streaming), on
+ * caller-held arrays: d_f_in = f_i^k(x, t) and d_f_out = f_i^k(x, t + 1), both DEVICE arrays [component][q][N] of
+ * cfg->compute_dtype in the layout and meaning of lbm_get_populations / lbm_set_populations (post-stream values;
+ * cfg->store_dtype is ignored), distinct from each other.  The psi field K1 hands to K2 is held in a static device array
+ * of LBM_NOALLOC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until exit), so
+ *     n_components * nx * ny * nz * sizeof(compute dtype) <= LBM_NOALLOC_SCRATCH_BYTES      (2 MiB: 512 x 256 fp32 with two
+ *     components, 512 x 512 fp64, 64^3 fp64, 80^3 fp32),
+ * larger domains are refused with LBM_E_NOMEM.  Built for: D2Q9 / D3Q19, one or two components, BGK / MRT, both forcing
+ * schemes, body force, fully periodic domains without solid cells and the plain Shan-Chen force (anything else:
+ * LBM_E_UNSUPPORTED; bad pointers or configuration: LBM_E_INVALID).  Asynchronous on `stream`; two kernel launches; no
+ * cudaMalloc / cudaFree / allocating library call, no host synchronisation.
+ * ALL calls on a GPU share the one scratch array: calls whose kernels may overlap on that GPU (different streams without
+ * ordering between them, several host threads or processes' contexts are separate copies) RACE on it -- order them.  The
+ * array keeps the previous call's contents; every word K2 reads is written by K1 of the same call, so nothing needs
+ * clearing.  lbm_noalloc_last_error() returns the calling thread's message for the last failing lbm_step_noalloc. */
+#define LBM_NOALLOC_SCRATCH_BYTES (2u << 20)
+LBM_API int lbm_step_noalloc(const lbm_config_t* cfg, const void* d_f_in, void* d_f_out, lbm_stream_t stream);
+LBM_API size_t lbm_noalloc_max_scratch_bytes(void);
+LBM_API const char* lbm_noalloc_last_error(void);
+
 /* Lattice tables: q, e[q][3], w[q], opposite[q].  Host pointers; any may be NULL. */
 LBM_API int lbm_get_lattice(int lattice, int* q, int* e, double* w, int* opposite);
 

@@ -80,6 +80,9 @@ _SIGNATURES = {
     "lbm_halo_bytes": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "lbm_export_halo": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "lbm_import_halo": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
+    "lbm_step_noalloc": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "lbm_noalloc_max_scratch_bytes": (C.c_size_t, []),
+    "lbm_noalloc_last_error": (C.c_char_p, []),
     "lbm_hot_path": (C.c_int, [C.c_void_p]),
     "lbm_steps_done": (C.c_int64, [C.c_void_p]),
     "lbm_kernel_launches": (C.c_int64, [C.c_void_p]),
@@ -387,6 +390,29 @@ class LBM:
     @property
     def kernel_launches(self) -> int:
         return int(self.L.lbm_kernel_launches(self.h))
+
+
+def step_noalloc(wl: dict, f_in, f_out, stream=None) -> None:
+    """lbm_step_noalloc (include/lbm.h): one time step f_in -> f_out on caller-held device tensors [nc][q][N] of the
+    compute dtype (the arrays get_populations_device returns), with no handle, no workspace and no allocation: psi lives
+    in a static device array inside the library (noalloc_max_scratch_bytes()).  Calls that overlap on the GPU race on it."""
+    import torch
+    L = load_library()
+    cfg = make_config(wl)
+    want = torch.float32 if wl.get("compute_dtype", "f64") == "f32" else torch.float64
+    n = cfg.n_components * (9 if cfg.lattice == 0 else 19) * cfg.nx * cfg.ny * cfg.nz
+    for t in (f_in, f_out):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == want and t.numel() == n):
+            raise LBMError("step_noalloc: f_in / f_out must be contiguous CUDA tensors [nc][q][N] of the compute dtype")
+    s = stream if stream is not None else torch.cuda.current_stream(f_in.device)
+    with torch.cuda.device(f_in.device):
+        rc = L.lbm_step_noalloc(C.byref(cfg), C.c_void_p(f_in.data_ptr()), C.c_void_p(f_out.data_ptr()), C.c_void_p(s.cuda_stream))
+    if rc != LBM_OK:
+        raise LBMError(f"lbm_step_noalloc failed: {STATUS.get(rc, rc)}: {L.lbm_noalloc_last_error().decode()}")
+
+
+def noalloc_max_scratch_bytes() -> int:
+    return int(load_library().lbm_noalloc_max_scratch_bytes())
 
 
 def get_lattice(name: str):

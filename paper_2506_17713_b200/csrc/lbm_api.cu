@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -989,6 +990,120 @@ int halo_ready(lbm* h) {
 }
 }  // namespace
 
+// ================================================================== lbm_step_noalloc (include/lbm.h)
+// One time step (S1..S7, the two-pass arrangement K1 -> K2) on caller-held populations, for callers that may not allocate
+// device memory and hold no workspace: psi, the one field K1 hands to K2, lives in a file-scope device array.  Every GPU
+// that loads the library holds LBM_NOALLOC_SCRATCH_BYTES of it until exit.  In host code the array's name is only a
+// stand-in: the device address comes from cudaGetSymbolAddress (noalloc_scratch(), once per device) and is what the
+// kernels get.  The arrays are the exported ones (post-stream f_i(x, t), compute dtype, [component][q][N]); K2 therefore
+// reads its own cell and PUSHES (f_out[i][x + e_i] = f*_i(x)) where the resident kernels pull.  Same device functions
+// (density, psi_of_rho, moments, psi_sums_rows, force_and_velocity, collide) in the same order as K1 / K2 of lbm_hot.cuh.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[LBM_NOALLOC_SCRATCH_BYTES];
+
+template <class L, int NC, class CT>
+__global__ void __launch_bounds__(256) k_noalloc_moments(const __grid_constant__ KParams<CT> p, const CT* __restrict__ f_in,
+                                                         CT* __restrict__ psi) {
+    for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < p.N; id += gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            CT f[L::Q];
+            static_for<0, L::Q>([&](auto I) { f[I] = f_in[((long long)k * L::Q + I) * p.N + id]; });
+            psi[(long long)k * p.N + id] = psi_of_rho(p, k, density<L, CT>(f));
+        }
+    }
+}
+
+template <class L, int NC, class CT, int COLL>
+__global__ void __launch_bounds__(256) k_noalloc_step(const __grid_constant__ KParams<CT> p, const CT* __restrict__ f_in,
+                                                      const CT* __restrict__ psi, CT* __restrict__ f_out) {
+    for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < p.N; id += gridDim.x * blockDim.x) {
+        const Cell c = make_cell<L>(p, id);
+        CT f[NC][L::Q], rho[NC], j[NC][3];
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            static_for<0, L::Q>([&](auto I) { f[k][I] = f_in[((long long)k * L::Q + I) * p.N + id]; });
+            moments<L, CT>(f[k], rho[k], j[k]);
+        }
+        CT u[3] = {CT(0), CT(0), CT(0)}, du[NC][3], S[NC][3], pc[NC];
+#pragma unroll
+        for (int kp = 0; kp < NC; ++kp) {
+            const CT* ps = psi + (long long)kp * p.N + id;
+            auto rowfn = [&](auto DY, auto DZ, auto NX, CT (&t)[1], CT& left, CT& right) {
+                constexpr int dy = DY, dz = DZ;
+                t[0] = ps[nbr_offset<0, dy, dz>(c)];
+                if constexpr (NX != 0) {
+                    left = ps[nbr_offset<-1, dy, dz>(c)];
+                    right = ps[nbr_offset<1, dy, dz>(c)];
+                }
+            };
+            CT S1[3][1], pc1[1];
+            psi_sums_rows<L, CT, 1>(rowfn, S1, pc1);
+            S[kp][0] = S1[0][0]; S[kp][1] = S1[1][0]; S[kp][2] = S1[2][0];
+            pc[kp] = pc1[0];
+        }
+        force_and_velocity<NC, CT>(p, rho, j, S, pc, u, du);
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            collide<L, COLL, CT>(p, k, rho[k], u, du[k], f[k]);
+            CT* out = f_out + (long long)k * L::Q * p.N + id;
+            static_for<0, L::Q>([&](auto I) {
+                out[(long long)I * p.N + nbr_offset<L::E[I][0], L::E[I][1], L::E[I][2]>(c)] = f[k][I];
+            });
+        }
+    }
+}
+
+namespace {
+thread_local std::string g_noalloc_err;
+int noalloc_fail(int code, const std::string& what) {
+    g_noalloc_err = what;
+    return code;
+}
+// device address of the static scratch array on the CURRENT device, looked up once per device
+int noalloc_scratch(void** out) {
+    static std::mutex mu;
+    static void* ptr[64] = {nullptr};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return noalloc_fail(LBM_E_CUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+    if (dev < 0 || dev >= 64) return noalloc_fail(LBM_E_UNSUPPORTED, "lbm_step_noalloc: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        void* q = nullptr;
+        e = cudaGetSymbolAddress(&q, g_noalloc_scratch);
+        if (e != cudaSuccess || !q) {
+            cudaGetLastError();
+            return noalloc_fail(LBM_E_CUDA, std::string("cudaGetSymbolAddress(g_noalloc_scratch): ") + cudaGetErrorString(e));
+        }
+        ptr[dev] = q;
+    }
+    *out = ptr[dev];
+    return LBM_OK;
+}
+
+template <class L, int NC, class CT, int COLL>
+cudaError_t noalloc_launch(const KParams<CT>& p, const void* f_in, void* scratch, void* f_out, cudaStream_t stream) {
+    const unsigned blocks = (unsigned)std::min<long long>(((long long)p.N + 255) / 256, 148LL * 32);
+    k_noalloc_moments<L, NC, CT><<<blocks, 256, 0, stream>>>(p, static_cast<const CT*>(f_in), static_cast<CT*>(scratch));
+    k_noalloc_step<L, NC, CT, COLL><<<blocks, 256, 0, stream>>>(p, static_cast<const CT*>(f_in), static_cast<const CT*>(scratch),
+                                                              static_cast<CT*>(f_out));
+    return cudaGetLastError();
+}
+template <class CT>
+cudaError_t noalloc_dispatch(const lbm_config_t& c, const KParams<CT>& p, const void* f_in, void* scratch, void* f_out,
+                             cudaStream_t stream) {
+    auto with_l = [&](auto Ltag, auto NC, auto COLL) {
+        using L = decltype(Ltag);
+        return noalloc_launch<L, NC, CT, COLL>(p, f_in, scratch, f_out, stream);
+    };
+    auto with_nc = [&](auto Ltag, auto COLL) {
+        return c.n_components == 1 ? with_l(Ltag, IC<1>{}, COLL) : with_l(Ltag, IC<2>{}, COLL);
+    };
+    auto with_coll = [&](auto Ltag) { return c.collision == LBM_MRT ? with_nc(Ltag, IC<1>{}) : with_nc(Ltag, IC<0>{}); };
+    return c.lattice == LBM_D2Q9 ? with_coll(D2Q9{}) : with_coll(D3Q19{});
+}
+}  // namespace
+
 extern "C" {
 
 size_t lbm_workspace_bytes(const lbm_config_t* cfg) {
@@ -1523,6 +1638,64 @@ int lbm_import_halo(lbm_t* h, int side, int width, const void* d_buf) {
     if (rc) return rc;
     if ((rc = halo_ready(h))) return rc;
     return halo_copy(h, g, side == 0 ? 0 : g.nl - (long long)width, const_cast<void*>(d_buf), false);
+}
+
+size_t lbm_noalloc_max_scratch_bytes(void) { return (size_t)LBM_NOALLOC_SCRATCH_BYTES; }
+const char* lbm_noalloc_last_error(void) { return g_noalloc_err.c_str(); }
+
+int lbm_step_noalloc(const lbm_config_t* cfg, const void* d_f_in, void* d_f_out, lbm_stream_t stream) {
+    g_noalloc_err.clear();
+    int rc = check_config(cfg);
+    if (rc != LBM_OK) return noalloc_fail(rc, "lbm_step_noalloc: invalid configuration");
+    const lbm_config_t& c = *cfg;
+    const int d = c.lattice == LBM_D2Q9 ? 2 : 3;
+    for (int a = 0; a < d; ++a)
+        if (!c.periodic[a]) return noalloc_fail(LBM_E_UNSUPPORTED, "lbm_step_noalloc: fully periodic domains only (no faces, no solid mask)");
+    if (c.flags & LBM_FLAG_NO_COLLIDE) return noalloc_fail(LBM_E_UNSUPPORTED, "lbm_step_noalloc: LBM_FLAG_NO_COLLIDE is not built");
+    if (c.zc_A[0] != 0.0 || c.st_kappa[0] != 0.0 || (c.n_components > 1 && (c.zc_A[1] != 0.0 || c.st_kappa[1] != 0.0)))
+        return noalloc_fail(LBM_E_UNSUPPORTED, "lbm_step_noalloc: plain Shan-Chen force only (no Zhang-Chen weight, no surface-tension source)");
+    const size_t cb = dtype_bytes(c.compute_dtype);
+    const size_t N = (size_t)c.nx * c.ny * c.nz;
+    const size_t need = (size_t)c.n_components * N * cb;
+    if (need > (size_t)LBM_NOALLOC_SCRATCH_BYTES)
+        return noalloc_fail(LBM_E_NOMEM, "lbm_step_noalloc: psi of this domain needs " + std::to_string(need) +
+                                             " bytes, the static scratch array holds " + std::to_string((size_t)LBM_NOALLOC_SCRATCH_BYTES) +
+                                             " (n_components * nx * ny * nz * sizeof(compute dtype) must not exceed it)");
+    if (!d_f_in || !d_f_out || d_f_in == d_f_out || ((uintptr_t)d_f_in % cb) != 0 || ((uintptr_t)d_f_out % cb) != 0)
+        return noalloc_fail(LBM_E_INVALID, "lbm_step_noalloc: f_in / f_out must be distinct device arrays aligned to the compute dtype");
+    void* scratch = nullptr;
+    if ((rc = noalloc_scratch(&scratch))) return rc;
+    // the kernel parameter block through the same code as the resident path: a handle-shaped record on the host stack
+    lbm t = lbm();
+    t.cfg = c;
+    t.q = q_of(c.lattice);
+    t.d = d;
+    t.N = (int)N;
+    t.plane = (long long)N;
+    t.sbytes = cb;
+    t.cbytes = cb;
+    t.ws = static_cast<char*>(scratch);
+    std::memset(&t.cv, 0, sizeof t.cv);
+    t.nbsolid = 0;
+    t.nfluid = (int)N;
+    t.nbr_stride = 0;
+    t.snbr_stride = 0;
+    t.force_rho = false;
+    for (int f = 0; f < 6; ++f) {
+        t.face_kind[f] = LBM_FACE_PERIODIC;
+        t.face_rho[f][0] = t.face_rho[f][1] = 1.0;
+        t.face_u[f][0] = t.face_u[f][1] = t.face_u[f][2] = 0.0;
+    }
+    cudaError_t e;
+    if (c.compute_dtype == LBM_F32) {
+        const KParams<float> p = make_params<float>(&t, 0, 0);
+        e = noalloc_dispatch<float>(c, p, d_f_in, scratch, d_f_out, static_cast<cudaStream_t>(stream));
+    } else {
+        const KParams<double> p = make_params<double>(&t, 0, 0);
+        e = noalloc_dispatch<double>(c, p, d_f_in, scratch, d_f_out, static_cast<cudaStream_t>(stream));
+    }
+    if (e != cudaSuccess) return noalloc_fail(LBM_E_CUDA, std::string("lbm_step_noalloc launch: ") + cudaGetErrorString(e));
+    return LBM_OK;
 }
 
 int lbm_hot_path(const lbm_t* h) { return h ? h->last_path : LBM_E_INVALID; }
