@@ -94,7 +94,8 @@ enum lbm_face_kind { LBM_FACE_PERIODIC = 0, LBM_FACE_WALL = 1, LBM_FACE_VELOCITY
 
 /* Tuning knobs.  NOT part of the ABI: environment variables read once, in lbm_create, for measurements and tests; no other
  * call reads the environment.  LBM_TUNE_FUSED_MCHUNK=<planes marched per CTA of the one-pass kernels>, LBM_TUNE_NO_EQ (run
- * k_fused_ws where k_fused_eq would apply), LBM_TUNE_EQ_HALF=0|1 (tile width of k_fused_eq), LBM_TUNE_LIST=0|1 and
+ * k_fused_ws where k_fused_eq would apply), LBM_TUNE_EQ_HALF=0|1 (tile width of k_fused_eq), LBM_TUNE_EQ_SPLIT=0|1|2 (k_fused_eq_split off / late / early
+ * take), LBM_TUNE_LIST=0|1 and
  * LBM_TUNE_COMPACT=0 (list / fluid-compact mode of the two-pass path on masked domains), LBM_TUNE_BRICK="bx,by,bz" (order of
  * the fluid-cell list), LBM_TUNE_NO_SNBR, LBM_TUNE_NO_PDL / LBM_TUNE_NO_GRAPH / LBM_TUNE_NO_COOP (plain launches on small
  * domains).  Results never depend on them beyond rounding order (none changes any arithmetic). */
@@ -292,7 +293,7 @@ enum lbm_path {
     LBM_PATH_RESERVED_2 = 2,        /* (round 1's lock-step one-pass kernel; removed) */
     LBM_PATH_ONE_PASS_WS = 3,       /* K2F k_fused_ws (warp-specialised, bulk asynchronous copies) */
     LBM_PATH_TWO_PASS_COMPACT = 4,  /* K1 (+K1b) + K2 on the fluid-compact layout (at most a quarter of the cells fluid) */
-    LBM_PATH_ONE_PASS_EQ = 5,       /* K2F k_fused_eq (row pipelines; one component, BGK with tau = 1) */
+    LBM_PATH_ONE_PASS_EQ = 5,       /* K2F k_fused_eq / k_fused_eq_split (row pipelines; one component, BGK with tau = 1) */
     LBM_PATH_TWO_PASS_PERSISTENT = 6 /* K1 | K1b | K2 as phases of one persistent cooperative kernel (small domains, n >= 2) */
 };
 LBM_API int lbm_hot_path(const lbm_t* h);

@@ -37,6 +37,7 @@ struct Tune {
     int compact = -1;      // LBM_TUNE_COMPACT=0: keep the dense layout where compact mode would apply
     int eq = -1;           // LBM_TUNE_NO_EQ=1 -> 0: k_fused_ws where k_fused_eq would apply
     int eq_half = -1;      // LBM_TUNE_EQ_HALF: force full-width (0) / half-width (1) tiles of k_fused_eq
+    int eq_split = -1;     // LBM_TUNE_EQ_SPLIT: k_fused_eq_split off (0) / on with late (1) / early (2) take; -1: chosen per domain
     bool no_snbr = false;  // LBM_TUNE_NO_SNBR: K1b of the compact mode on the dense rho field
     bool no_pdl = false;   // LBM_TUNE_NO_PDL / LBM_TUNE_NO_GRAPH / LBM_TUNE_NO_COOP: plain launches on small domains
     bool no_graph = false;
@@ -50,6 +51,7 @@ struct Tune {
         t.compact = geti("LBM_TUNE_COMPACT", -1);
         t.eq = std::getenv("LBM_TUNE_NO_EQ") ? 0 : -1;
         t.eq_half = geti("LBM_TUNE_EQ_HALF", -1);
+        t.eq_split = geti("LBM_TUNE_EQ_SPLIT", -1);
         t.no_snbr = std::getenv("LBM_TUNE_NO_SNBR") != nullptr;
         t.no_pdl = std::getenv("LBM_TUNE_NO_PDL") != nullptr;
         t.no_graph = std::getenv("LBM_TUNE_NO_GRAPH") != nullptr;
@@ -77,6 +79,7 @@ struct lbm {
     int fmchunk;         // planes marched per CTA
     bool use_fused;      // decided in prepare()
     bool eq_half;        // k_fused_eq with half-width tiles and two CTAs per SM
+    int eq_split;        // 0: k_fused_eq; 1 / 2: k_fused_eq_split (front / back warps per row) with late / early take
     bool feq;            // one component, BGK, tau = 1: the collision result is f_eq(rho, u' + du) (k_fused_eq applies)
     int last_path;       // lbm_hot_path: what the last lbm_step ran
     // launch-bound (small) domains: GRAPH_STEPS time steps captured once into a CUDA graph and replayed
@@ -652,7 +655,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.list = (h->use_list && (op == OP_MOMENTS || (op == OP_STEP && !a.zc))) ? (h->is_compact ? 2 : 1) : 0;
     a.a0 = a0; a.a1 = a1; a.a2 = a2; a.i0 = i0;
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;   // (also read by the compact kernels)
-    a.eq = h->feq ? (h->eq_half ? 2 : 1) : 0;
+    a.eq = h->feq ? (h->eq_split ? 2 + h->eq_split : (h->eq_half ? 2 : 1)) : 0;
     a.pdl = h->pdl ? 1 : 0;
     a.used_kernel = op == OP_FUSED ? &h->last_path : nullptr;
     a.stream = h->stream;
@@ -731,6 +734,22 @@ void plan_fused(lbm* h) {
         const long long cols = (long long)((c.nx + txf - 1) / txf) * ((c.ny + h->fshape.ty - 1) / h->fshape.ty);
         h->eq_half = h->tune.eq_half >= 0 ? h->tune.eq_half != 0
                                           : h->fshape.vec >= 2 && ((uf < 0.9 && uh > uf + 0.05) || cols < nsm / 4);
+    }
+    // k_fused_eq_split (fp32 compute and storage): front / back warps per row.  Measured, ms per step, k_fused_eq (full /
+    // half width) | split, late take | split, early take:   128^3 .0767 / .0733 | .0721 | .0688;  256^3 .550 | .511 | .447;
+    // 320^3 1.138 | 1.074 | 1.019;  384^3 1.659 | 1.65 | 1.78;  448^3 2.980 | 2.824 | 2.749;  512^3 3.90 | 4.02 | 4.14;
+    // 416^3 (paper's case) 2.714 / 2.59 | 2.491 | 2.406.  The split kernel loses where the tiles are full in x AND the
+    // columns fill the GPU (384^3: 144 columns, 512^3: 256): neighbouring tiles drift apart and re-read their shared halo
+    // rows from DRAM (lbm_fused_eq2.cuh) -- k_fused_eq stays there; elsewhere the split kernel with the early take runs.
+    // A forced tile width (LBM_TUNE_EQ_HALF) keeps k_fused_eq.
+    h->eq_split = 0;
+    if (h->feq && c.compute_dtype == LBM_F32 && c.store_dtype == LBM_F32 && h->fshape.vec == 4) {
+        const int txf = 32 * h->fshape.vec;
+        const long long cols = (long long)((c.nx + txf - 1) / txf) * ((c.ny + h->fshape.ty - 1) / h->fshape.ty);
+        const bool keep = c.nx % txf == 0 && 16 * cols >= 15LL * nsm;
+        if (h->tune.eq_split >= 0) h->eq_split = std::min(h->tune.eq_split, 2);
+        else if (h->tune.eq_half < 0) h->eq_split = keep ? 0 : 2;
+        if (h->eq_split) h->eq_half = false;
     }
     const bool half = h->feq && h->eq_half;
     const int tx = 32 * h->fshape.vec / (half ? 2 : 1);
@@ -1156,6 +1175,7 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->use_fused = false;
     h->feq = false;
     h->eq_half = false;
+    h->eq_split = 0;
     h->last_path = LBM_PATH_NONE;
     h->gexec = nullptr;
     h->gcur = 0;

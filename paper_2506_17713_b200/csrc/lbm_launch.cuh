@@ -5,6 +5,7 @@
 #include <cstdlib>
 #include "lbm_fused_ws.cuh"
 #include "lbm_fused_eq.cuh"
+#include "lbm_fused_eq2.cuh"
 #include "lbm_compact.cuh"
 #include "lbm_small.cuh"
 
@@ -31,7 +32,7 @@ struct LaunchArgs {
     void* a2;
     int i0;              // op-specific integer (OP_FUSED: planes marched per CTA)
     int eq;              // OP_FUSED: one component, BGK, tau = 1 (f* is an equilibrium): the row-pipeline kernel k_fused_eq applies
-                         //           (2: with half-width tiles and two CTAs per SM)
+                         //           (2: with half-width tiles and two CTAs per SM; 3 / 4: k_fused_eq_split, late / early take)
     int* used_kernel;    // OP_FUSED, out: the lbm_path value of the kernel that ran
     int wref;            // OP_FUSED: rho_ref != 0 (populations stored shifted by w_i rho_ref)
     int pdl;             // OP_MOMENTS / OP_VIRTUAL / OP_STEP (dense mapping): programmatic dependent launch (pdl_begin)
@@ -297,7 +298,29 @@ cudaError_t launch(const LaunchArgs& a) {
                                 done = true;
                             }
                         };
-                        if (a.eq == 2) {
+                        // k_fused_eq_split: front / back warps per row (lbm_fused_eq2.cuh); fp32 compute and storage
+                        auto go_split = [&](auto EARLY, auto WREF) {
+                            constexpr int vec = fused_shape<L, CT, ST, NC>().vec, ty = fused_shape<L, CT, ST, NC>().ty;
+                            if constexpr (NC == 1 && C_ == 0 && vec == 4 && sizeof(CT) == 4 && sizeof(ST) == 4) {
+                                using T = EqSplitTile<L, CT, ST, vec, ty>;
+                                auto kern = k_fused_eq_split<L, CT, ST, vec, ty, (EARLY != 0), (WREF != 0)>;
+                                static int ready[16] = {0};
+                                if (!usable(kern, ready, T::SMEM, T::REGS_NEEDED, T::THREADS)) return;
+                                dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + ty - 1) / ty),
+                                       (unsigned)((p.nz + a.i0 - 1) / a.i0));
+                                kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0);
+                                if (a.used_kernel) *a.used_kernel = 5;  // LBM_PATH_ONE_PASS_EQ
+                                done = true;
+                            }
+                        };
+                        if (a.eq == 3 || a.eq == 4) {
+                            if (a.eq == 4) { if (a.wref) go_split(IC<1>{}, IC<1>{}); else go_split(IC<1>{}, IC<0>{}); }
+                            else { if (a.wref) go_split(IC<0>{}, IC<1>{}); else go_split(IC<0>{}, IC<0>{}); }
+                            if (!done) {   // not built for this dtype combination: the single-warp row pipeline
+                                if (a.wref) go_eq(IC<fs.vec>{}, IC<1>{}, IC<1>{});
+                                else go_eq(IC<fs.vec>{}, IC<1>{}, IC<0>{});
+                            }
+                        } else if (a.eq == 2) {
                             if (a.wref) go_eq(IC<fs.vec / 2>{}, IC<2>{}, IC<1>{});
                             else go_eq(IC<fs.vec / 2>{}, IC<2>{}, IC<0>{});
                         } else if (a.eq == 1) {

@@ -21,6 +21,16 @@ def one_pass(wl):
     return w
 
 
+def select_eq_kernel(monkeypatch, kernel):
+    """k_fused_eq at full / half tile width, or k_fused_eq_split (built for fp32 compute and storage; other dtypes fall
+    back to k_fused_eq) with the late / early take -- by the tuning knobs of include/lbm.h"""
+    if kernel.startswith("k_fused_eq_split"):
+        monkeypatch.setenv("LBM_TUNE_EQ_SPLIT", "2" if kernel.endswith("early") else "1")
+    else:
+        monkeypatch.setenv("LBM_TUNE_EQ_SPLIT", "0")
+        monkeypatch.setenv("LBM_TUNE_EQ_HALF", "1" if kernel == "k_fused_eq_half" else "0")
+
+
 def run_three(wl, inp, steps, oracle_wl=None):
     """oracle, K2F and the two-pass path on the same inputs; returns populations of each."""
     o = make_oracle(oracle_wl or wl, inp)
@@ -41,14 +51,14 @@ def run_three(wl, inp, steps, oracle_wl=None):
             [g2.get_populations(k) for k in range(o.nc)], o)
 
 
-@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_ws"])
+@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_eq_split_late", "k_fused_eq_split_early", "k_fused_ws"])
 @pytest.mark.parametrize("dims", [(128, 24, 20), (132, 9, 11), (4, 3, 2), (260, 8, 5), (8, 35, 3)])
 def test_d3q19_fp64_ragged_tiles(dims, kernel, monkeypatch):
     monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "7")   # several marching chunks, ragged last one
     if kernel == "k_fused_ws":                          # the general kernel where k_fused_eq would apply
         monkeypatch.setenv("LBM_TUNE_NO_EQ", "1")
     else:
-        monkeypatch.setenv("LBM_TUNE_EQ_HALF", "1" if kernel == "k_fused_eq_half" else "0")
+        select_eq_kernel(monkeypatch, kernel)
     wl, _ = W.config5(16, "f64")
     wl.update(nx=dims[0], ny=dims[1], nz=dims[2])
     inp = small_inputs(wl, 21, 0.05, 0.3)
@@ -58,12 +68,28 @@ def test_d3q19_fp64_ragged_tiles(dims, kernel, monkeypatch):
     assert_parity(f2, f1, fluid, 1e-13, relative=False)   # same arithmetic in the same order as K2
 
 
-@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_ws"])
+@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_split_late", "k_fused_eq_split_early"])
+@pytest.mark.parametrize("dims", [(128, 24, 20), (132, 9, 11), (4, 3, 2), (260, 8, 5), (8, 35, 3), (200, 17, 9)])
+def test_d3q19_fp32_ragged_tiles(dims, kernel, monkeypatch):
+    """fp32 compute and storage (what k_fused_eq_split is built for): ragged tiles in x and y, chunks with a ragged tail,
+    domains smaller than a tile or a half row; against the fp64 oracle and the two-pass path."""
+    monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "7")
+    select_eq_kernel(monkeypatch, kernel)
+    wl, _ = W.config5(16, "f32")
+    wl.update(nx=dims[0], ny=dims[1], nz=dims[2])
+    inp = small_inputs(wl, 22, 0.05, 0.3)
+    fo, f1, f2, o = run_three(wl, inp, 30, oracle_wl=with_dtype(wl, "f64"))
+    fluid = np.ones(o.N, bool)
+    assert_parity(fo, f1, fluid, TOL32, relative=True)
+    assert_parity(f2, f1, fluid, 2e-6, relative=True)    # same arithmetic as K1 / K2 (fp32: up to contraction of a*b+c)
+
+
+@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_eq_split_late", "k_fused_eq_split_early", "k_fused_ws"])
 def test_config5_fp32_100_steps(kernel, monkeypatch):
     if kernel == "k_fused_ws":
         monkeypatch.setenv("LBM_TUNE_NO_EQ", "1")
     else:
-        monkeypatch.setenv("LBM_TUNE_EQ_HALF", "1" if kernel == "k_fused_eq_half" else "0")
+        select_eq_kernel(monkeypatch, kernel)
     wl, inp = W.config5(48, "f32")
     fo, f1, f2, o = run_three(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
     fluid = np.ones(o.N, bool)
