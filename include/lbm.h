@@ -294,7 +294,9 @@ enum lbm_path {
     LBM_PATH_ONE_PASS_WS = 3,       /* K2F k_fused_ws (warp-specialised, bulk asynchronous copies) */
     LBM_PATH_TWO_PASS_COMPACT = 4,  /* K1 (+K1b) + K2 on the fluid-compact layout (at most a quarter of the cells fluid) */
     LBM_PATH_ONE_PASS_EQ = 5,       /* K2F k_fused_eq / k_fused_eq_split (row pipelines; one component, BGK with tau = 1) */
-    LBM_PATH_TWO_PASS_PERSISTENT = 6 /* K1 | K1b | K2 as phases of one persistent cooperative kernel (small domains, n >= 2) */
+    LBM_PATH_TWO_PASS_PERSISTENT = 6, /* K1 | K1b | K2 as phases of one persistent cooperative kernel (small domains, n >= 2) */
+    LBM_PATH_ONE_PASS_TILE = 7       /* small 2-D domains, n >= 2: one persistent kernel, rho / psi recomputed on a ring around each
+                                        CTA's tile, one grid barrier per step (k_steps_tile) */
 };
 LBM_API int lbm_hot_path(const lbm_t* h);
 

@@ -378,10 +378,10 @@ class LBM:
 
     @property
     def hot_path(self) -> str:
-        """What the most recent step() launched: 'two_pass', 'one_pass_ws', 'one_pass_eq', 'two_pass_compact' or
-        'two_pass_persistent'."""
+        """What the most recent step() launched: 'two_pass', 'one_pass_ws', 'one_pass_eq', 'two_pass_compact',
+        'two_pass_persistent' or 'one_pass_tile'."""
         return {0: "none", 1: "two_pass", 3: "one_pass_ws", 4: "two_pass_compact", 5: "one_pass_eq",
-                6: "two_pass_persistent"}[int(self.L.lbm_hot_path(self.h))]
+                6: "two_pass_persistent", 7: "one_pass_tile"}[int(self.L.lbm_hot_path(self.h))]
 
     @property
     def steps_done(self) -> int:

@@ -42,6 +42,7 @@ struct Tune {
     bool no_pdl = false;   // LBM_TUNE_NO_PDL / LBM_TUNE_NO_GRAPH / LBM_TUNE_NO_COOP: plain launches on small domains
     bool no_graph = false;
     bool no_coop = false;
+    bool no_tile = false;  // LBM_TUNE_NO_TILE: small 2-D domains on k_steps_coop / graph replay instead of k_steps_tile
     int brick[3] = {32, 16, 16};   // LBM_TUNE_BRICK="bx,by,bz": bricks of the fluid list's order (bx = 0: ascending cell index)
     static Tune from_env() {
         Tune t;
@@ -56,6 +57,7 @@ struct Tune {
         t.no_pdl = std::getenv("LBM_TUNE_NO_PDL") != nullptr;
         t.no_graph = std::getenv("LBM_TUNE_NO_GRAPH") != nullptr;
         t.no_coop = std::getenv("LBM_TUNE_NO_COOP") != nullptr;
+        t.no_tile = std::getenv("LBM_TUNE_NO_TILE") != nullptr;
         if (const char* e = std::getenv("LBM_TUNE_BRICK")) {
             int v[3] = {0, 1, 1};
             if (std::sscanf(e, "%d,%d,%d", &v[0], &v[1], &v[2]) >= 1) { t.brick[0] = v[0]; t.brick[1] = std::max(1, v[1]); t.brick[2] = std::max(1, v[2]); }
@@ -87,6 +89,7 @@ struct lbm {
     int gcur;            // buffer parity the graph was captured at
     int64_t glaunches;   // kernels per replay
     bool gvalid, gfailed;
+    bool tile_failed;    // k_steps_tile does not apply (3-D, more tiles than resident CTAs, no cooperative launch)
     bool coop_failed;    // the cooperative launch of the persistent small-domain kernel is not available
     bool initialized, has_solid, bnd, dirty, force_rho;
     int nbsolid;
@@ -1183,6 +1186,7 @@ int lbm_create(const lbm_config_t* cfg, void* d_workspace, size_t workspace_byte
     h->gvalid = false;
     h->gfailed = false;
     h->coop_failed = false;
+    h->tile_failed = false;
     h->initialized = false;
     h->has_solid = false;
     h->dirty = true;
@@ -1340,6 +1344,21 @@ int lbm_step(lbm_t* h, int n) {
     // the launch latency between them
     const bool ext_force = h->cfg.zc_A[0] != 0.0 || h->cfg.st_kappa[0] != 0.0 ||
                            (h->cfg.n_components > 1 && (h->cfg.zc_A[1] != 0.0 || h->cfg.st_kappa[1] != 0.0));
+    if (small && n >= 2 && h->d == 2 && !h->profiling && !h->tile_failed && !h->tune.no_coop && !h->tune.no_tile && !h->use_fused &&
+        !h->use_list && !ext_force && !(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) {
+        // 2-D: rho / psi recomputed on a ring around each CTA's tile, ONE grid barrier per step (k_steps_tile)
+        unsigned* ctr = reinterpret_cast<unsigned*>(h->ws + h->cv.counter + 64);
+        CU(cudaMemsetAsync(ctr, 0, sizeof(unsigned), h->stream));
+        rc = do_launch(h, OP_TILE, nullptr, nullptr, ctr, n);
+        if (rc == LBM_OK) {
+            h->cur ^= (n & 1);
+            h->steps += n;
+            h->last_path = LBM_PATH_ONE_PASS_TILE;
+            return LBM_OK;
+        }
+        h->tile_failed = true;
+        h->err.clear();
+    }
     if (small && n >= 2 && !h->profiling && !h->coop_failed && !h->tune.no_coop && !h->use_fused && !h->use_list && !ext_force) {
         unsigned* ctr = reinterpret_cast<unsigned*>(h->ws + h->cv.counter + 64);
         CU(cudaMemsetAsync(ctr, 0, sizeof(unsigned), h->stream));

@@ -15,7 +15,8 @@ enum Op { OP_MOMENTS = 0, OP_VIRTUAL = 1, OP_STEP = 2, OP_INIT = 3, OP_EXPORT_MA
           OP_BUILD_NBR = 9 /* a0 = dense -> extended index map, a2 = table */, OP_FILL_SOLID = 10,
           OP_PACK_C = 11 /* dense -> compact layout */, OP_UNPACK_C = 12 /* compact -> dense */,
           OP_BUILD_SNBR = 13 /* a0 = dense -> extended index map, a2 = table of the boundary solids */,
-          OP_COOP = 14 /* i0 = time steps, a2 = barrier counter (zeroed): the persistent kernel of small domains */ };
+          OP_COOP = 14 /* i0 = time steps, a2 = barrier counter (zeroed): the persistent kernel of small domains */,
+          OP_TILE = 15 /* same arguments: the tiled persistent kernel of small 2-D domains (one barrier per step) */ };
 
 struct LaunchArgs {
     int op;
@@ -196,6 +197,48 @@ cudaError_t launch(const LaunchArgs& a) {
                     });
                 });
             });
+            if (err != cudaSuccess) { cudaGetLastError(); return err; }
+            break;
+        }
+        case OP_TILE: {
+            // k_steps_tile (lbm_small.cuh): one CTA per TW x TH tile, all resident, one grid barrier per step
+            cudaError_t err = cudaErrorNotSupported;
+            if constexpr (L::D == 2) {
+                with_nc([&](auto NC) {
+                    with_bnd([&](auto B) {
+                        auto with_coll = [&](auto fn) {
+                            if (a.coll == 0) fn(IC<0>{});
+                            else if (a.coll == 1) fn(IC<1>{});
+                        };
+                        with_coll([&](auto C_) {
+                            int dev = 0, nsm = 0, coop = 0;
+                            cudaGetDevice(&dev);
+                            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+                            cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+                            if (!coop) return;
+                            auto go = [&](auto TW_, auto TH_) {
+                                constexpr int TW = TW_, TH = TH_;
+                                using T = SmallTile<TW, TH, (B != 0)>;
+                                auto kern = k_steps_tile<L, NC, CT, ST, C_, (B != 0), TW, TH>;
+                                const size_t smem = T::template smem<CT>(NC);
+                                const int g = ((p.nx + TW - 1) / TW) * ((p.ny + TH - 1) / TH);
+                                int per_sm = 0;
+                                if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+                                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T::NT, smem) != cudaSuccess || g > nsm * per_sm) return false;
+                                int nsteps = a.i0;
+                                unsigned* ctr = static_cast<unsigned*>(a.a2);
+                                void* args[] = {const_cast<void*>(static_cast<const void*>(&p)), &nsteps, &ctr};
+                                err = cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kern), dim3((unsigned)g), dim3(T::NT), args, smem, a.stream);
+                                return true;
+                            };
+                            // small tiles while they give every cell a thread on one CTA per SM, larger ones otherwise
+                            const long long small_tiles = (long long)((p.nx + 15) / 16) * ((p.ny + 15) / 16);
+                            if (small_tiles <= nsm) { if (go(IC<16>{}, IC<16>{})) return; }
+                            go(IC<32>{}, IC<16>{});
+                        });
+                    });
+                });
+            }
             if (err != cudaSuccess) { cudaGetLastError(); return err; }
             break;
         }

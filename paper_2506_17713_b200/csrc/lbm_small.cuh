@@ -161,4 +161,185 @@ __global__ void __launch_bounds__(256) k_steps_coop(const __grid_constant__ KPar
     }
 }
 
+// ------------------------------------------------------------------ k_steps_tile: ONE grid barrier per time step (D2Q9)
+// The three phases of a step need two exchanges between SMs because psi(rho) of the new time level must be known at the
+// eight neighbours before the force can be formed (and, next to walls, the virtual density of a boundary solid averages
+// rho over ITS fluid neighbours, Eq. 17: a reach of two cells).  Here a CTA owns a TW x TH tile, one cell per thread, and
+// recomputes rho and psi on a ring of H cells around it (H = 1 on fully periodic domains without solid cells, 2 otherwise)
+// from the populations themselves -- the one-pass idea of K2F (lbm_fused_ws.cuh) on a 2-D tile:
+//
+//   A  every position of the (TW + 2H) x (TH + 2H) region: pull, rho (S1), psi (S3) into shared memory; the thread keeps
+//      the populations of its own cell in registers
+//   B  (masked / walled domains) solid positions of the inner ring: virtual density from the shared rho (S2, Eq. 17), psi
+//   C  own cell: j, force from the shared psi (S4, S5), collide (S6), boundary rules and store (S7)
+//   -- grid barrier, buffers swapped --
+//
+// so a step costs one trip through L2 and one grid barrier instead of two or three of each.  The ring is 27 % (H = 1,
+// 16 x 16) to 41 % (H = 2, 32 x 16) more pulls, all L2 hits.  Same device functions and the same order of every sum as
+// k_moments_v / k_virtual_density / k_step_v: bit-identical to the plain launches (tested).  The global rho / psi fields
+// are not written (every entry point that reads them refreshes them first, as after the one-pass kernels).
+// Positions beyond a non-periodic face do not exist: the neighbour offsets of an edge cell are clamped as in make_cell.
+template <int TW, int TH, bool BND>
+struct SmallTile {
+    static constexpr int H = BND ? 2 : 1;
+    static constexpr int RW = TW + 2 * H, RH = TH + 2 * H;
+    static constexpr int NT = TW * TH;
+    static constexpr int NPOS = RW * RH;
+    static constexpr int NBORDER = NPOS - NT;
+    template <class CT> static constexpr size_t smem(int nc) {
+        return (size_t)NPOS * (sizeof(CT) * nc * (BND ? 2 : 1) + 4 + (BND ? 4 : 0));
+    }
+};
+
+template <class L, int NC, class CT, class ST, int COLL, bool BND, int TW, int TH>
+__global__ void __launch_bounds__(TW * TH, (TW * TH >= 512 ? 2 : 1)) k_steps_tile(const __grid_constant__ KParams<CT> p, int nsteps, unsigned* ctr) {
+    static_assert(L::D == 2 && COLL != 2, "2-D lattices, with a collision");
+    using T = SmallTile<TW, TH, BND>;
+    constexpr int H = T::H, RW = T::RW, NPOS = T::NPOS, NT = T::NT, Q = L::Q;
+    extern __shared__ __align__(16) unsigned char smem_t[];
+    CT* psi_s = reinterpret_cast<CT*>(smem_t);                              // [NC][NPOS]
+    CT* rho_s = psi_s + (BND ? NC * NPOS : 0);                              // [NC][NPOS] (walled domains)
+    int* gid_s = reinterpret_cast<int*>(psi_s + (BND ? 2 : 1) * NC * NPOS); // global cell of a position, -1: none
+    uint32_t* fl_s = reinterpret_cast<uint32_t*>(gid_s + NPOS);             // its flags (walled domains)
+
+    const int tid = threadIdx.x;
+    const int tiles_x = (p.nx + TW - 1) / TW;
+    const int x0 = (int)(blockIdx.x % tiles_x) * TW, y0 = (int)(blockIdx.x / tiles_x) * TH;
+    // position -> global cell (wrap on periodic axes; nothing beyond a non-periodic face), once
+    for (int pos = tid; pos < NPOS; pos += NT) {
+        int gx = x0 + pos % RW - H, gy = y0 + pos / RW - H;
+        bool ok = true;
+        if (gx < 0) { if (p.periodic[0]) gx += p.nx; else ok = false; }
+        else if (gx >= p.nx) { if (p.periodic[0]) gx -= p.nx; else ok = false; }
+        if (gy < 0) { if (p.periodic[1]) gy += p.ny; else ok = false; }
+        else if (gy >= p.ny) { if (p.periodic[1]) gy -= p.ny; else ok = false; }
+        ok = ok && gx >= 0 && gx < p.nx && gy >= 0 && gy < p.ny;     // (domains narrower than the ring)
+        const int g = ok ? gy * p.nx + gx : -1;
+        gid_s[pos] = g;
+        if constexpr (BND) fl_s[pos] = ok ? __ldg(p.flags + g) : SOLID_BIT;
+    }
+    __syncthreads();
+    // the thread's own cell and the border positions it serves in phase A
+    const int tx = tid % TW, ty = tid / TW;
+    const int own = (ty + H) * RW + tx + H;
+    const bool mine = x0 + tx < p.nx && y0 + ty < p.ny;                   // ragged tiles: the position may still serve as a ring
+    const int own_g = gid_s[own];
+    uint32_t own_fl = 0;
+    if constexpr (BND) own_fl = fl_s[own];
+    const bool own_fluid = mine && !(own_fl & SOLID_BIT);
+    Cell oc = make_cell<L>(p, own_g < 0 ? 0 : own_g);
+    // local neighbour offsets of the own cell (clamped at non-periodic faces like oc.sxm ..)
+    const int lxm = oc.sxm != 0 ? -1 : 0, lxp = oc.sxp != 0 ? 1 : 0, lym = oc.sym != 0 ? -RW : 0, lyp = oc.syp != 0 ? RW : 0;
+    auto border_pos = [&](int b) {   // b-th position of the region outside the tile
+        if (b < H * RW) return b;                                                 // rows above
+        b -= H * RW;
+        if (b < TH * 2 * H) { const int r = b / (2 * H), c = b % (2 * H); return (H + r) * RW + (c < H ? c : TW + c); }
+        b -= TH * 2 * H;
+        return (H + TH) * RW + b;                                                 // rows below
+    };
+
+    const ST* fa = static_cast<const ST*>(p.f_in);
+    ST* fb = static_cast<ST*>(p.f_out);
+    unsigned target = 0;
+    for (int s = 0; s < nsteps; ++s) {
+        // ---- A: rho, psi of every position; own populations stay in registers
+        CT f[NC][Q];
+        auto moments_at = [&](int pos, const Cell& c, uint32_t fl, CT (&fk)[Q], int k) {
+            pull_cg<L, CT, ST, BND>(p, fa, c, fl, k, fk);
+            const CT r = density<L, CT>(fk);
+            psi_s[k * NPOS + pos] = psi_of_rho(p, k, r);
+            if constexpr (BND) rho_s[k * NPOS + pos] = r;
+        };
+        if (own_g >= 0 && !(own_fl & SOLID_BIT)) {
+#pragma unroll
+            for (int k = 0; k < NC; ++k) moments_at(own, oc, own_fl, f[k], k);
+        }
+        for (int b = tid; b < T::NBORDER; b += NT) {
+            const int pos = border_pos(b);
+            const int g = gid_s[pos];
+            uint32_t fl = 0;
+            if constexpr (BND) fl = fl_s[pos];
+            if (g < 0 || (fl & SOLID_BIT)) continue;
+            const Cell c = make_cell<L>(p, g);
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {
+                CT fk[Q];
+                moments_at(pos, c, fl, fk, k);
+            }
+        }
+        __syncthreads();
+        // ---- B: virtual density at the solid positions of the tile and its inner ring (S2, Eq. 17; as k_virtual_density)
+        if constexpr (BND) {
+            if (p.nbsolid > 0) {
+                constexpr int IW = TW + 2, IH = TH + 2;
+                for (int q = tid; q < IW * IH; q += NT) {
+                    const int pos = (H - 1 + q / IW) * RW + (H - 1) + q % IW;
+                    const int g = gid_s[pos];
+                    if (g < 0 || !(fl_s[pos] & SOLID_BIT)) continue;
+                    const Cell c = make_cell<L>(p, g);
+                    const int dxm = c.sxm != 0 ? -1 : 0, dxp = c.sxp != 0 ? 1 : 0, dym = c.sym != 0 ? -RW : 0, dyp = c.syp != 0 ? RW : 0;
+                    CT num[NC], den = CT(0);
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) num[k] = CT(0);
+                    static_for<1, Q>([&](auto I) {
+                        constexpr int i = I;
+                        constexpr CT w = CT(L::WN[i]) / CT(L::WD);
+                        constexpr int ex = L::E[i][0], ey = L::E[i][1];
+                        const int nb = pos + (ex > 0 ? dxp : (ex < 0 ? dxm : 0)) + (ey > 0 ? dyp : (ey < 0 ? dym : 0));
+                        if (!(fl_s[nb] & SOLID_BIT)) {
+                            den += w;
+#pragma unroll
+                            for (int k = 0; k < NC; ++k) num[k] += w * rho_s[k * NPOS + nb];
+                        }
+                    });
+                    if (den > CT(0)) {
+#pragma unroll
+                        for (int k = 0; k < NC; ++k) {
+                            CT rs = p.wet_phi[k] * (num[k] / den) - p.wet_drho[k];
+                            rs = rs < p.wet_lo[k] ? p.wet_lo[k] : rs;
+                            rs = rs > p.wet_hi[k] ? p.wet_hi[k] : rs;
+                            psi_s[k * NPOS + pos] = psi_of_rho(p, k, rs);
+                        }
+                    }
+                }
+                __syncthreads();
+            }
+        }
+        // ---- C: own cell (as k_step_v)
+        if (own_fluid) {
+            CT rho[NC], j[NC][3];
+#pragma unroll
+            for (int k = 0; k < NC; ++k) moments<L, CT>(f[k], rho[k], j[k]);
+            CT u[3] = {CT(0), CT(0), CT(0)}, du[NC][3];
+            CT S[NC][3], pc[NC];
+#pragma unroll
+            for (int kp = 0; kp < NC; ++kp) {
+                const CT* ps = psi_s + kp * NPOS + own;
+                auto rowfn = [&](auto DY, auto DZ, auto NX, CT (&t)[1], CT& left, CT& right) {
+                    constexpr int dy = DY;
+                    const CT* row = ps + (dy > 0 ? lyp : (dy < 0 ? lym : 0));
+                    t[0] = row[0];
+                    if constexpr (NX != 0) { left = row[lxm]; right = row[lxp]; }
+                };
+                CT S1[3][1], pc1[1];
+                psi_sums_rows<L, CT, 1>(rowfn, S1, pc1);
+                S[kp][0] = S1[0][0]; S[kp][1] = S1[1][0]; S[kp][2] = S1[2][0];
+                pc[kp] = pc1[0];
+            }
+            force_and_velocity<NC, CT>(p, rho, j, S, pc, u, du);
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {
+                collide<L, COLL, CT>(p, k, rho[k], u, du[k], f[k]);
+                if constexpr (BND) {
+                    if (own_fl & FACEBC_BIT) apply_face_rules<L, CT>(p, oc, k, u, f[k]);
+                }
+                ST* out = fb + (long long)k * Q * p.plane + oc.id;
+                static_for<0, Q>([&](auto I) { Conv<CT, ST>::st(out + (long long)I * p.plane, f[k][I] - p.wref[I]); });
+            }
+        }
+        grid_barrier(ctr, target, gridDim.x);       // (its __syncthreads also fences the shared fields for the next step)
+        const ST* t_ = fa; fa = fb; fb = const_cast<ST*>(t_);
+    }
+}
+
 }  // namespace lbmk

@@ -494,9 +494,14 @@ def test_persistent_kernel_and_graph_replay_match_plain_launches(monkeypatch):
     for wl, inp in (W.config1(64, "f64"), W.config2(64, 32, "f32", wall=3), (wl3, inp3), W.config3(16, "f32")):
         dt = np.float64 if wl["compute_dtype"] == "f64" else np.float32
         outs = {}
-        for how in ("persistent", "graph", "plain"):
-            if how == "persistent":
+        for how in ("tile", "persistent", "graph", "plain"):
+            if how == "tile" and wl["lattice"] != "D2Q9":
+                continue
+            monkeypatch.delenv("LBM_TUNE_NO_TILE", raising=False)
+            if how in ("tile", "persistent"):
                 monkeypatch.delenv("LBM_TUNE_NO_COOP", raising=False)
+                if how == "persistent":
+                    monkeypatch.setenv("LBM_TUNE_NO_TILE", "1")
             else:
                 monkeypatch.setenv("LBM_TUNE_NO_COOP", "1")
             if wl is wl3:
@@ -510,14 +515,16 @@ def test_persistent_kernel_and_graph_replay_match_plain_launches(monkeypatch):
             s.step(40)           # graph reused
             torch.cuda.synchronize()
             assert s.steps_done == 118
-            assert s.hot_path == ("two_pass_persistent" if how == "persistent" else "two_pass"), (wl["name"], how, s.hot_path)
-            if how == "persistent":
+            assert s.hot_path == {"tile": "one_pass_tile", "persistent": "two_pass_persistent"}.get(how, "two_pass"), (wl["name"], how, s.hot_path)
+            if how in ("tile", "persistent"):
                 assert s.kernel_launches < 40            # three step calls, a handful of preprocessing kernels
             outs[how] = [s.get_populations(k) for k in range(s.nc)]
             monkeypatch.delenv("LBM_TUNE_LIST", raising=False)
         for k in range(len(outs["plain"])):
             assert np.array_equal(outs["persistent"][k], outs["plain"][k]), (wl["name"], k)
             assert np.array_equal(outs["graph"][k], outs["plain"][k]), (wl["name"], k)
+            if "tile" in outs:
+                assert np.array_equal(outs["tile"][k], outs["plain"][k]), (wl["name"], k)
 
 
 # ------------------------------------------------------------------ NEXT-2: surface-tension control (Eq. 14-16, D2Q9 MRT)
