@@ -216,25 +216,26 @@ cudaError_t launch(const LaunchArgs& a) {
                             cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
                             cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
                             if (!coop) return;
-                            auto go = [&](auto TW_, auto TH_) {
-                                constexpr int TW = TW_, TH = TH_;
-                                using T = SmallTile<TW, TH, (B != 0)>;
-                                auto kern = k_steps_tile<L, NC, CT, ST, C_, (B != 0), TW, TH>;
-                                const size_t smem = T::template smem<CT>(NC);
+                            auto go = [&](auto TW_, auto TH_, auto CPT_) {
+                                constexpr int TW = TW_, TH = TH_, CPT = CPT_;
+                                using T = SmallTile<TW, TH, CPT, (B != 0)>;
+                                auto kern = k_steps_tile<L, NC, CT, ST, C_, (B != 0), TW, TH, CPT>;
+                                const size_t smem = T::template smem<CT>(NC, L::Q);
                                 const int g = ((p.nx + TW - 1) / TW) * ((p.ny + TH - 1) / TH);
+                                if (g > nsm) return false;          // one CTA per SM, all resident
                                 int per_sm = 0;
                                 if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
-                                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T::NT, smem) != cudaSuccess || g > nsm * per_sm) return false;
+                                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T::NT, smem) != cudaSuccess || per_sm < 1) return false;
                                 int nsteps = a.i0;
                                 unsigned* ctr = static_cast<unsigned*>(a.a2);
                                 void* args[] = {const_cast<void*>(static_cast<const void*>(&p)), &nsteps, &ctr};
                                 err = cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kern), dim3((unsigned)g), dim3(T::NT), args, smem, a.stream);
                                 return true;
                             };
-                            // small tiles while they give every cell a thread on one CTA per SM, larger ones otherwise
-                            const long long small_tiles = (long long)((p.nx + 15) / 16) * ((p.ny + 15) / 16);
-                            if (small_tiles <= nsm) { if (go(IC<16>{}, IC<16>{})) return; }
-                            go(IC<32>{}, IC<16>{});
+                            // the smallest tile that gives every SM at most one CTA, one cell per thread
+                            if (go(IC<16>{}, IC<16>{}, IC<1>{})) return;
+                            if (go(IC<32>{}, IC<16>{}, IC<1>{})) return;
+                            go(IC<64>{}, IC<16>{}, IC<1>{});
                         });
                     });
                 });

@@ -179,33 +179,40 @@ __global__ void __launch_bounds__(256) k_steps_coop(const __grid_constant__ KPar
 // k_moments_v / k_virtual_density / k_step_v: bit-identical to the plain launches (tested).  The global rho / psi fields
 // are not written (every entry point that reads them refreshes them first, as after the one-pass kernels).
 // Positions beyond a non-periodic face do not exist: the neighbour offsets of an edge cell are clamped as in make_cell.
-template <int TW, int TH, bool BND>
+// TW x TH cells per CTA, CPT of them per thread
+template <int TW, int TH, int CPT, bool BND>
 struct SmallTile {
     static constexpr int H = BND ? 2 : 1;
     static constexpr int RW = TW + 2 * H, RH = TH + 2 * H;
-    static constexpr int NT = TW * TH;
+    static constexpr int NCELL = TW * TH;
     static constexpr int NPOS = RW * RH;
-    static constexpr int NBORDER = NPOS - NT;
-    template <class CT> static constexpr size_t smem(int nc) {
-        return (size_t)NPOS * (sizeof(CT) * nc * (BND ? 2 : 1) + 4 + (BND ? 4 : 0));
+    // one cell per thread: extra threads for the ring where they fit, so that every pull of phase A is in flight at once
+    static constexpr int NT = CPT == 1 ? ((NPOS + 31) / 32 * 32 <= 1024 ? (NPOS + 31) / 32 * 32 : NCELL) : NCELL / CPT;
+    static constexpr int NR = (NPOS + NT - 1) / NT;       // positions per thread in phase A (the first CPT are its own cells)
+    static_assert(NCELL % CPT == 0 && NT % 32 == 0 && NT <= 1024, "whole warps");
+    template <class CT> static constexpr size_t smem(int nc, int q) {
+        return (size_t)NPOS * (sizeof(CT) * nc * (BND ? 2 : 1) + 4 + (BND ? 4 : 0) + 4 * q);
     }
 };
 
-template <class L, int NC, class CT, class ST, int COLL, bool BND, int TW, int TH>
-__global__ void __launch_bounds__(TW * TH, (TW * TH >= 512 ? 2 : 1)) k_steps_tile(const __grid_constant__ KParams<CT> p, int nsteps, unsigned* ctr) {
+template <class L, int NC, class CT, class ST, int COLL, bool BND, int TW, int TH, int CPT>
+__global__ void __launch_bounds__((SmallTile<TW, TH, CPT, BND>::NT), 1)
+k_steps_tile(const __grid_constant__ KParams<CT> p, int nsteps, unsigned* ctr) {
     static_assert(L::D == 2 && COLL != 2, "2-D lattices, with a collision");
-    using T = SmallTile<TW, TH, BND>;
-    constexpr int H = T::H, RW = T::RW, NPOS = T::NPOS, NT = T::NT, Q = L::Q;
+    using T = SmallTile<TW, TH, CPT, BND>;
+    constexpr int H = T::H, RW = T::RW, NPOS = T::NPOS, NT = T::NT, NR = T::NR, Q = L::Q;
     extern __shared__ __align__(16) unsigned char smem_t[];
     CT* psi_s = reinterpret_cast<CT*>(smem_t);                              // [NC][NPOS]
     CT* rho_s = psi_s + (BND ? NC * NPOS : 0);                              // [NC][NPOS] (walled domains)
     int* gid_s = reinterpret_cast<int*>(psi_s + (BND ? 2 : 1) * NC * NPOS); // global cell of a position, -1: none
     uint32_t* fl_s = reinterpret_cast<uint32_t*>(gid_s + NPOS);             // its flags (walled domains)
+    uint32_t* src_s = fl_s + (BND ? NPOS : 0);                              // [Q][NPOS] element a pull reads, within a component
 
     const int tid = threadIdx.x;
     const int tiles_x = (p.nx + TW - 1) / TW;
     const int x0 = (int)(blockIdx.x % tiles_x) * TW, y0 = (int)(blockIdx.x / tiles_x) * TH;
     // position -> global cell (wrap on periodic axes; nothing beyond a non-periodic face), once
+    int has_solid = 0;
     for (int pos = tid; pos < NPOS; pos += NT) {
         int gx = x0 + pos % RW - H, gy = y0 + pos / RW - H;
         bool ok = true;
@@ -216,61 +223,84 @@ __global__ void __launch_bounds__(TW * TH, (TW * TH >= 512 ? 2 : 1)) k_steps_til
         ok = ok && gx >= 0 && gx < p.nx && gy >= 0 && gy < p.ny;     // (domains narrower than the ring)
         const int g = ok ? gy * p.nx + gx : -1;
         gid_s[pos] = g;
-        if constexpr (BND) fl_s[pos] = ok ? __ldg(p.flags + g) : SOLID_BIT;
+        uint32_t fl = 0;
+        if constexpr (BND) {
+            fl = ok ? __ldg(p.flags + g) : SOLID_BIT;
+            fl_s[pos] = fl;
+            has_solid |= ok && (fl & SOLID_BIT) != 0;
+        }
+        // S7 read side as pull(): stored_i(x - e_i), or stored_ibar(x) on a flagged link -- the element index, once
+        if (ok && !(fl & SOLID_BIT)) {
+            const Cell c = make_cell<L>(p, g);
+            static_for<0, Q>([&](auto I) {
+                constexpr int i = I;
+                constexpr int ib = opposite<L>(i);
+                long long e = (long long)i * p.plane + g;
+                if constexpr (i > 0) {
+                    if (BND && ((fl >> i) & 1u)) e = (long long)ib * p.plane + g;
+                    else e += nbr_offset<-L::E[i][0], -L::E[i][1], -L::E[i][2]>(c);
+                }
+                src_s[i * NPOS + pos] = (uint32_t)e;
+            });
+        }
     }
-    __syncthreads();
-    // the thread's own cell and the border positions it serves in phase A
-    const int tx = tid % TW, ty = tid / TW;
-    const int own = (ty + H) * RW + tx + H;
-    const bool mine = x0 + tx < p.nx && y0 + ty < p.ny;                   // ragged tiles: the position may still serve as a ring
-    const int own_g = gid_s[own];
-    uint32_t own_fl = 0;
-    if constexpr (BND) own_fl = fl_s[own];
-    const bool own_fluid = mine && !(own_fl & SOLID_BIT);
-    Cell oc = make_cell<L>(p, own_g < 0 ? 0 : own_g);
-    // local neighbour offsets of the own cell (clamped at non-periodic faces like oc.sxm ..)
-    const int lxm = oc.sxm != 0 ? -1 : 0, lxp = oc.sxp != 0 ? 1 : 0, lym = oc.sym != 0 ? -RW : 0, lyp = oc.syp != 0 ? RW : 0;
-    auto border_pos = [&](int b) {   // b-th position of the region outside the tile
+    // phase B is skipped by CTAs whose region holds no solid cell
+    const int any_solid = __syncthreads_or(has_solid);     // (also the barrier between writing and reading gid_s / fl_s)
+    const bool do_b = BND && any_solid && p.nbsolid > 0;
+    // the e-th position of the region: the cells of the tile first (row by row), then the ring around it
+    auto pos_of = [&](int e) {
+        if (e < T::NCELL) return (e / TW + H) * RW + e % TW + H;
+        int b = e - T::NCELL;
         if (b < H * RW) return b;                                                 // rows above
         b -= H * RW;
         if (b < TH * 2 * H) { const int r = b / (2 * H), c = b % (2 * H); return (H + r) * RW + (c < H ? c : TW + c); }
         b -= TH * 2 * H;
         return (H + TH) * RW + b;                                                 // rows below
     };
+    // this thread's positions in phase A; bit r of `live`: a fluid cell of the domain sits there
+    int posr[NR];
+    unsigned live = 0, mine = 0;
+#pragma unroll
+    for (int r = 0; r < NR; ++r) {
+        const int e = tid + r * NT;
+        posr[r] = e < NPOS ? pos_of(e) : 0;
+        bool ok = e < NPOS && gid_s[posr[r]] >= 0;
+        if constexpr (BND) ok = ok && !(fl_s[posr[r]] & SOLID_BIT);
+        if (ok) live |= 1u << r;
+        // own cell of the tile AND inside the domain as such (a ragged tile's positions beyond the edge only serve as ring)
+        if (r < CPT && ok && e < T::NCELL && x0 + e % TW < p.nx && y0 + e / TW < p.ny) mine |= 1u << r;
+    }
 
     const ST* fa = static_cast<const ST*>(p.f_in);
     ST* fb = static_cast<ST*>(p.f_out);
     unsigned target = 0;
     for (int s = 0; s < nsteps; ++s) {
-        // ---- A: rho, psi of every position; own populations stay in registers
-        CT f[NC][Q];
-        auto moments_at = [&](int pos, const Cell& c, uint32_t fl, CT (&fk)[Q], int k) {
-            pull_cg<L, CT, ST, BND>(p, fa, c, fl, k, fk);
-            const CT r = density<L, CT>(fk);
-            psi_s[k * NPOS + pos] = psi_of_rho(p, k, r);
-            if constexpr (BND) rho_s[k * NPOS + pos] = r;
-        };
-        if (own_g >= 0 && !(own_fl & SOLID_BIT)) {
+        // ---- A: pull at every position of the thread (all loads in flight together), then rho, psi into shared memory;
+        //         the populations of the own cells stay in registers
+        CT f[CPT][NC][Q];
+        static_for<0, NR>([&](auto R) {
+            constexpr int r = R;
+            if ((live >> r) & 1u) {
+                const int pos = posr[r];
 #pragma unroll
-            for (int k = 0; k < NC; ++k) moments_at(own, oc, own_fl, f[k], k);
-        }
-        for (int b = tid; b < T::NBORDER; b += NT) {
-            const int pos = border_pos(b);
-            const int g = gid_s[pos];
-            uint32_t fl = 0;
-            if constexpr (BND) fl = fl_s[pos];
-            if (g < 0 || (fl & SOLID_BIT)) continue;
-            const Cell c = make_cell<L>(p, g);
+                for (int k = 0; k < NC; ++k) {
+                    CT tmp[Q];
+                    const ST* base = fa + (long long)k * Q * p.plane;
+                    static_for<0, Q>([&](auto I) { tmp[I] = CgLoad<CT, ST>::ld(base + src_s[I * NPOS + pos]) + p.wref[I]; });
+                    const CT rr = density<L, CT>(tmp);
+                    psi_s[k * NPOS + pos] = psi_of_rho(p, k, rr);
+                    if constexpr (BND) rho_s[k * NPOS + pos] = rr;
+                    if constexpr (r < CPT) {
 #pragma unroll
-            for (int k = 0; k < NC; ++k) {
-                CT fk[Q];
-                moments_at(pos, c, fl, fk, k);
+                        for (int i = 0; i < Q; ++i) f[r][k][i] = tmp[i];
+                    }
+                }
             }
-        }
+        });
         __syncthreads();
         // ---- B: virtual density at the solid positions of the tile and its inner ring (S2, Eq. 17; as k_virtual_density)
         if constexpr (BND) {
-            if (p.nbsolid > 0) {
+            if (do_b) {
                 constexpr int IW = TW + 2, IH = TH + 2;
                 for (int q = tid; q < IW * IH; q += NT) {
                     const int pos = (H - 1 + q / IW) * RW + (H - 1) + q % IW;
@@ -305,11 +335,19 @@ __global__ void __launch_bounds__(TW * TH, (TW * TH >= 512 ? 2 : 1)) k_steps_til
                 __syncthreads();
             }
         }
-        // ---- C: own cell (as k_step_v)
-        if (own_fluid) {
+        // ---- C: own cells (as k_step_v)
+#pragma unroll
+        for (int r = 0; r < CPT; ++r) {
+            if (!((mine >> r) & 1u)) continue;
+            const int own = posr[r];
+            uint32_t own_fl = 0;
+            if constexpr (BND) own_fl = fl_s[own];
+            const Cell oc = make_cell<L>(p, gid_s[own]);
+            // local neighbour offsets (clamped at non-periodic faces like oc.sxm ..)
+            const int lxm = oc.sxm != 0 ? -1 : 0, lxp = oc.sxp != 0 ? 1 : 0, lym = oc.sym != 0 ? -RW : 0, lyp = oc.syp != 0 ? RW : 0;
             CT rho[NC], j[NC][3];
 #pragma unroll
-            for (int k = 0; k < NC; ++k) moments<L, CT>(f[k], rho[k], j[k]);
+            for (int k = 0; k < NC; ++k) moments<L, CT>(f[r][k], rho[k], j[k]);
             CT u[3] = {CT(0), CT(0), CT(0)}, du[NC][3];
             CT S[NC][3], pc[NC];
 #pragma unroll
@@ -329,12 +367,12 @@ __global__ void __launch_bounds__(TW * TH, (TW * TH >= 512 ? 2 : 1)) k_steps_til
             force_and_velocity<NC, CT>(p, rho, j, S, pc, u, du);
 #pragma unroll
             for (int k = 0; k < NC; ++k) {
-                collide<L, COLL, CT>(p, k, rho[k], u, du[k], f[k]);
+                collide<L, COLL, CT>(p, k, rho[k], u, du[k], f[r][k]);
                 if constexpr (BND) {
-                    if (own_fl & FACEBC_BIT) apply_face_rules<L, CT>(p, oc, k, u, f[k]);
+                    if (own_fl & FACEBC_BIT) apply_face_rules<L, CT>(p, oc, k, u, f[r][k]);
                 }
                 ST* out = fb + (long long)k * Q * p.plane + oc.id;
-                static_for<0, Q>([&](auto I) { Conv<CT, ST>::st(out + (long long)I * p.plane, f[k][I] - p.wref[I]); });
+                static_for<0, Q>([&](auto I) { Conv<CT, ST>::st(out + (long long)I * p.plane, f[r][k][I] - p.wref[I]); });
             }
         }
         grid_barrier(ctr, target, gridDim.x);       // (its __syncthreads also fences the shared fields for the next step)

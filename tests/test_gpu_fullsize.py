@@ -165,10 +165,10 @@ def test_config5_256_fp64_sampled_cells():
 
 def test_config2_512x256_every_cell_100_steps():
     """config 2 at its full size is small enough for the oracle: every population of every cell after 100 steps, in the
-    launch configuration bench.py times (fp32, CUDA-graph replay of the three kernels)"""
+    launch configuration bench.py times (fp32, the tiled persistent kernel k_steps_tile: one grid barrier per step)"""
     wl, inp = W.config2(512, 256, "f32")
     o, g, fo, fg = run_pair(wl, inp, 100, oracle_wl=with_dtype(wl, "f64"))
-    assert g.hot_path == "two_pass"
+    assert g.hot_path == "one_pass_tile"
     assert_parity(fo, fg, fluid_mask(inp, o.N), TOL32, relative=True)
     ro, _, _ = o.get_macroscopic()
     rg, _, _ = g.get_macroscopic()
