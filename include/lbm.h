@@ -280,7 +280,9 @@ enum lbm_kernel_id {
     LBM_K_VIRTUAL = 1, /* K1b: virtual density at boundary solids */
     LBM_K_STEP = 2,    /* K2: fused stream + force + collide + boundary (two-pass path) */
     LBM_K_FUSED = 3,   /* K2F: one-pass kernel (moments + psi of the halo recomputed in the tile) */
-    LBM_K_COUNT = 4
+    LBM_K_PERSISTENT = 4, /* the persistent kernels of small domains (k_steps_tile / k_steps_coop): one launch makes n time
+                             steps; its time is recorded as a whole and `launches` counts the n steps */
+    LBM_K_COUNT = 5
 };
 LBM_API int lbm_set_profiling(lbm_t* h, int enable);
 LBM_API int lbm_get_kernel_times(lbm_t* h, double* ms_total, int64_t* launches);

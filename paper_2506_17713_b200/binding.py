@@ -25,7 +25,7 @@ COLLISIONS = {"BGK": 0, "MRT": 1}
 FORCINGS = {"EDM": 0, "SHIFT": 1}
 DTYPES = {"f16": 0, "f32": 1, "f64": 2}
 FACE_KINDS = {"PERIODIC": 0, "WALL": 1, "VELOCITY": 2, "PRESSURE": 3}
-KERNEL_IDS = {"moments": 0, "virtual": 1, "step": 2, "fused": 3}
+KERNEL_IDS = {"moments": 0, "virtual": 1, "step": 2, "fused": 3, "persistent": 4}
 FLAG_NO_COLLIDE = 1
 FLAG_TWO_PASS = 2
 FLAG_ONE_PASS = 4

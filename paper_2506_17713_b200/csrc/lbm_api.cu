@@ -112,7 +112,7 @@ struct lbm {
     // measurement only (lbm_set_profiling): event pairs around hot-loop kernels
     bool profiling;
     std::vector<cudaEvent_t> ev_pool;
-    struct EvPair { int kid; cudaEvent_t a, b; };
+    struct EvPair { int kid; int n; cudaEvent_t a, b; };   // n: time steps the bracketed launch made
     std::vector<EvPair> ev_pending;
     double k_ms[LBM_K_COUNT];
     int64_t k_cnt[LBM_K_COUNT];
@@ -603,7 +603,7 @@ int prof_drain(lbm* h) {
         float ms = 0.f;
         CU(cudaEventElapsedTime(&ms, pr.a, pr.b));
         h->k_ms[pr.kid] += ms;
-        h->k_cnt[pr.kid] += 1;
+        h->k_cnt[pr.kid] += pr.n;
         h->ev_pool.push_back(pr.a);
         h->ev_pool.push_back(pr.b);
     }
@@ -630,6 +630,7 @@ int hot_launch(lbm* h, int op, int kid) {
     if (h->ev_pending.size() >= 2048) { int rc = prof_drain(h); if (rc) return rc; }
     lbm::EvPair pr;
     pr.kid = kid;
+    pr.n = 1;
     int rc = prof_event(h, &pr.a);
     if (rc) return rc;
     rc = do_launch(h, op, nullptr, nullptr, nullptr, i0, -1, -1);
@@ -1344,12 +1345,30 @@ int lbm_step(lbm_t* h, int n) {
     // the launch latency between them
     const bool ext_force = h->cfg.zc_A[0] != 0.0 || h->cfg.st_kappa[0] != 0.0 ||
                            (h->cfg.n_components > 1 && (h->cfg.zc_A[1] != 0.0 || h->cfg.st_kappa[1] != 0.0));
-    if (small && n >= 2 && h->d == 2 && !h->profiling && !h->tile_failed && !h->tune.no_coop && !h->tune.no_tile && !h->use_fused &&
+    // (while profiling, a persistent launch is bracketed as a whole and counted as n steps of LBM_K_PERSISTENT)
+    auto persistent_launch = [&](int op, unsigned* ctr) -> int {
+        lbm::EvPair pr;
+        pr.kid = LBM_K_PERSISTENT;
+        pr.n = n;
+        int r;
+        if (h->profiling && (r = prof_event(h, &pr.a))) return r;
+        r = do_launch(h, op, nullptr, nullptr, ctr, n);
+        if (r != LBM_OK) {
+            if (h->profiling) h->ev_pool.push_back(pr.a);
+            return r;
+        }
+        if (h->profiling) {
+            if ((r = prof_event(h, &pr.b))) return r;
+            h->ev_pending.push_back(pr);
+        }
+        return LBM_OK;
+    };
+    if (small && n >= 2 && h->d == 2 && !h->tile_failed && !h->tune.no_coop && !h->tune.no_tile && !h->use_fused &&
         !h->use_list && !ext_force && !(h->cfg.flags & LBM_FLAG_NO_COLLIDE)) {
         // 2-D: rho / psi recomputed on a ring around each CTA's tile, ONE grid barrier per step (k_steps_tile)
         unsigned* ctr = reinterpret_cast<unsigned*>(h->ws + h->cv.counter + 64);
         CU(cudaMemsetAsync(ctr, 0, sizeof(unsigned), h->stream));
-        rc = do_launch(h, OP_TILE, nullptr, nullptr, ctr, n);
+        rc = persistent_launch(OP_TILE, ctr);
         if (rc == LBM_OK) {
             h->cur ^= (n & 1);
             h->steps += n;
@@ -1359,10 +1378,10 @@ int lbm_step(lbm_t* h, int n) {
         h->tile_failed = true;
         h->err.clear();
     }
-    if (small && n >= 2 && !h->profiling && !h->coop_failed && !h->tune.no_coop && !h->use_fused && !h->use_list && !ext_force) {
+    if (small && n >= 2 && !h->coop_failed && !h->tune.no_coop && !h->use_fused && !h->use_list && !ext_force) {
         unsigned* ctr = reinterpret_cast<unsigned*>(h->ws + h->cv.counter + 64);
         CU(cudaMemsetAsync(ctr, 0, sizeof(unsigned), h->stream));
-        rc = do_launch(h, OP_COOP, nullptr, nullptr, ctr, n);
+        rc = persistent_launch(OP_COOP, ctr);
         if (rc == LBM_OK) {
             h->cur ^= (n & 1);
             h->steps += n;
