@@ -233,6 +233,7 @@ cudaError_t launch(const LaunchArgs& a) {
                                 return true;
                             };
                             // the smallest tile that gives every SM at most one CTA, one cell per thread
+                            if (go(IC<8>{}, IC<8>{}, IC<1>{})) return;
                             if (go(IC<16>{}, IC<16>{}, IC<1>{})) return;
                             if (go(IC<32>{}, IC<16>{}, IC<1>{})) return;
                             go(IC<64>{}, IC<16>{}, IC<1>{});

@@ -260,6 +260,7 @@ k_steps_tile(const __grid_constant__ KParams<CT> p, int nsteps, unsigned* ctr) {
     // this thread's positions in phase A; bit r of `live`: a fluid cell of the domain sits there
     int posr[NR];
     unsigned live = 0, mine = 0;
+    unsigned lofs[CPT];                 // own cells: bits 0..3 = the neighbour at x-1, x+1, y-1, y+1 is another position
 #pragma unroll
     for (int r = 0; r < NR; ++r) {
         const int e = tid + r * NT;
@@ -268,7 +269,14 @@ k_steps_tile(const __grid_constant__ KParams<CT> p, int nsteps, unsigned* ctr) {
         if constexpr (BND) ok = ok && !(fl_s[posr[r]] & SOLID_BIT);
         if (ok) live |= 1u << r;
         // own cell of the tile AND inside the domain as such (a ragged tile's positions beyond the edge only serve as ring)
-        if (r < CPT && ok && e < T::NCELL && x0 + e % TW < p.nx && y0 + e / TW < p.ny) mine |= 1u << r;
+        if (r < CPT) {
+            lofs[r] = 0;
+            if (ok && e < T::NCELL && x0 + e % TW < p.nx && y0 + e / TW < p.ny) {
+                mine |= 1u << r;
+                const Cell c = make_cell<L>(p, gid_s[posr[r]]);
+                lofs[r] = (c.sxm != 0 ? 1u : 0u) | (c.sxp != 0 ? 2u : 0u) | (c.sym != 0 ? 4u : 0u) | (c.syp != 0 ? 8u : 0u);
+            }
+        }
     }
 
     const ST* fa = static_cast<const ST*>(p.f_in);
@@ -342,9 +350,10 @@ k_steps_tile(const __grid_constant__ KParams<CT> p, int nsteps, unsigned* ctr) {
             const int own = posr[r];
             uint32_t own_fl = 0;
             if constexpr (BND) own_fl = fl_s[own];
-            const Cell oc = make_cell<L>(p, gid_s[own]);
-            // local neighbour offsets (clamped at non-periodic faces like oc.sxm ..)
-            const int lxm = oc.sxm != 0 ? -1 : 0, lxp = oc.sxp != 0 ? 1 : 0, lym = oc.sym != 0 ? -RW : 0, lyp = oc.syp != 0 ? RW : 0;
+            // local neighbour offsets (clamped at non-periodic faces like Cell::sxm ..), packed before the step loop
+            const int lxm = -(int)((lofs[r] >> 0) & 1u), lxp = (int)((lofs[r] >> 1) & 1u);
+            const int lym = ((lofs[r] >> 2) & 1u) ? -RW : 0, lyp = ((lofs[r] >> 3) & 1u) ? RW : 0;
+            const int own_id = gid_s[own];
             CT rho[NC], j[NC][3];
 #pragma unroll
             for (int k = 0; k < NC; ++k) moments<L, CT>(f[r][k], rho[k], j[k]);
@@ -369,9 +378,9 @@ k_steps_tile(const __grid_constant__ KParams<CT> p, int nsteps, unsigned* ctr) {
             for (int k = 0; k < NC; ++k) {
                 collide<L, COLL, CT>(p, k, rho[k], u, du[k], f[r][k]);
                 if constexpr (BND) {
-                    if (own_fl & FACEBC_BIT) apply_face_rules<L, CT>(p, oc, k, u, f[r][k]);
+                    if (own_fl & FACEBC_BIT) apply_face_rules<L, CT>(p, make_cell<L>(p, own_id), k, u, f[r][k]);
                 }
-                ST* out = fb + (long long)k * Q * p.plane + oc.id;
+                ST* out = fb + (long long)k * Q * p.plane + own_id;
                 static_for<0, Q>([&](auto I) { Conv<CT, ST>::st(out + (long long)I * p.plane, f[r][k][I] - p.wref[I]); });
             }
         }
