@@ -98,7 +98,7 @@ enum lbm_face_kind { LBM_FACE_PERIODIC = 0, LBM_FACE_WALL = 1, LBM_FACE_VELOCITY
  * take), LBM_TUNE_LIST=0|1 and
  * LBM_TUNE_COMPACT=0 (list / fluid-compact mode of the two-pass path on masked domains), LBM_TUNE_BRICK="bx,by,bz" (order of
  * the fluid-cell list), LBM_TUNE_NO_SNBR, LBM_TUNE_NO_PDL / LBM_TUNE_NO_GRAPH / LBM_TUNE_NO_COOP (plain launches on small
- * domains).  Results never depend on them beyond rounding order (none changes any arithmetic). */
+ * domains), LBM_TUNE_NO_TILE (small 2-D domains on k_steps_coop / graph replay instead of k_steps_tile).  Results never depend on them beyond rounding order (none changes any arithmetic). */
 
 typedef struct {
     int32_t psi_kind; /* lbm_psi_kind */
@@ -182,7 +182,11 @@ LBM_API int lbm_init_fields(lbm_t* h, const void* const* rho, const void* u, int
  * Layout note: on a masked domain with at most a quarter of the cells fluid (and a plain Shan-Chen force) the steps
  * run on a fluid-compact copy of the populations (lbm_hot_path reports LBM_PATH_TWO_PASS_COMPACT); the first step
  * after, and the first export / import after such steps, each cost one extra copy kernel.  Results are bit-identical
- * to the dense layout; solid cells read back as f_eq(1,0), whatever lbm_set_populations had put there. */
+ * to the dense layout; solid cells read back as f_eq(1,0), whatever lbm_set_populations had put there.
+ * Small domains (n_components * cells <= 2^22) with n >= 2: all n steps run as ONE cooperative launch of a persistent
+ * kernel where the device allows it -- 2-D lattices on k_steps_tile (LBM_PATH_ONE_PASS_TILE: rho and psi recomputed on a
+ * ring around each CTA's tile, one grid barrier per step), others on k_steps_coop (LBM_PATH_TWO_PASS_PERSISTENT) --, else
+ * as CUDA-graph replays of 16 captured steps; bit-identical to n calls with n = 1, which launch the kernels one by one. */
 LBM_API int lbm_step(lbm_t* h, int n);
 
 /* S8: rho^k (virtual density at boundary solids, 0 inside solids), u = (sum_k j^k + 1/2 sum_k F^k)/sum_k rho^k
