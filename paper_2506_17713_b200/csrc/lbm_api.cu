@@ -10,6 +10,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
+#include <queue>
 #include <new>
 #include <string>
 #include <vector>
@@ -765,10 +766,40 @@ void plan_fused(lbm* h) {
     const long long slots = (long long)nsm * (half ? 2 : 1);   // CTAs resident at a time
     long long best_cost = -1;
     int mchunk = nm;
+    // ... with a ragged last x tile (k_fused_eq_split; 416 = 3.25 tiles) the CTAs are not equal -- a narrow tile moves fewer
+    // bytes and finishes earlier -- and "waves" no longer describes the schedule: the launch order is then played through
+    // (every CTA goes to the SM that is free first; cost of a CTA = (planes + 5) x (3/4 + 1/4 of the width fraction), the
+    // weighting that ranks the sweeps below best) and the chunk with the shortest makespan wins.  With equal tiles this IS
+    // waves x (planes + 5).  Measured, ms per step by planes per CTA: 416^3: 208 (the wave model's choice) 2.40, 139 2.55,
+    // 104 2.35, 84 2.34, 70 2.33, 60 2.26 (picked), 52 2.30, 35 2.29;  320^3: 107 1.156, 80 1.153, 54 1.018 (picked), 40 1.045;
+    // 448^3: 150 2.96, 90 2.81 (picked), 64 2.74, 56 2.77.
+    const int xt_all = (c.nx + tx - 1) / tx;
+    const bool ragged = h->eq_split != 0 && c.nx % tx != 0;
+    const long long ycols = tiles / xt_all;
     for (int nch = 1; nch <= std::max(1, nm / 8); ++nch) {
         const int mc = (nm + nch - 1) / nch;
-        const long long ctas = tiles * ((nm + mc - 1) / mc);
-        const long long cost = ((ctas + slots - 1) / slots) * (mc + 5);
+        const int nchunks = (nm + mc - 1) / mc;
+        const long long ctas = tiles * nchunks;
+        long long cost;
+        if (!ragged || ctas > 200000) {
+            cost = ((ctas + slots - 1) / slots) * (mc + 5);
+        } else {
+            std::priority_queue<long long, std::vector<long long>, std::greater<long long>> sm;
+            for (long long s_ = 0; s_ < slots; ++s_) sm.push(0);
+            long long makespan = 0;
+            for (int z = 0; z < nchunks; ++z) {
+                const long long planes = std::min(mc, nm - z * mc) + 5;
+                for (long long y = 0; y < ycols; ++y)
+                    for (int x = 0; x < xt_all; ++x) {
+                        const long long w = std::min(tx, c.nx - x * tx);           // cells of the row the tile covers
+                        const long long t = sm.top() + planes * (3 * tx + w);
+                        sm.pop();
+                        sm.push(t);
+                        makespan = std::max(makespan, t);
+                    }
+            }
+            cost = makespan;
+        }
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; mchunk = mc; }
     }
     if (h->tune.mchunk > 0) mchunk = std::max(1, std::min(nm, h->tune.mchunk));
