@@ -38,6 +38,7 @@ struct Tune {
     int compact = -1;      // LBM_TUNE_COMPACT=0: keep the dense layout where compact mode would apply
     int eq = -1;           // LBM_TUNE_NO_EQ=1 -> 0: k_fused_ws where k_fused_eq would apply
     int eq_half = -1;      // LBM_TUNE_EQ_HALF: force full-width (0) / half-width (1) tiles of k_fused_eq
+    int eq_ygroup = -1;    // LBM_TUNE_EQ_YGROUP: k_fused_eq_split launched per chunk of planes and per group of this many tile rows (0: one launch)
     int eq_split = -1;     // LBM_TUNE_EQ_SPLIT: k_fused_eq_split off (0) / on with late (1) / early (2) take; -1: chosen per domain
     bool no_snbr = false;  // LBM_TUNE_NO_SNBR: K1b of the compact mode on the dense rho field
     bool no_pdl = false;   // LBM_TUNE_NO_PDL / LBM_TUNE_NO_GRAPH / LBM_TUNE_NO_COOP: plain launches on small domains
@@ -54,6 +55,7 @@ struct Tune {
         t.eq = std::getenv("LBM_TUNE_NO_EQ") ? 0 : -1;
         t.eq_half = geti("LBM_TUNE_EQ_HALF", -1);
         t.eq_split = geti("LBM_TUNE_EQ_SPLIT", -1);
+        t.eq_ygroup = geti("LBM_TUNE_EQ_YGROUP", -1);
         t.no_snbr = std::getenv("LBM_TUNE_NO_SNBR") != nullptr;
         t.no_pdl = std::getenv("LBM_TUNE_NO_PDL") != nullptr;
         t.no_graph = std::getenv("LBM_TUNE_NO_GRAPH") != nullptr;
@@ -82,6 +84,7 @@ struct lbm {
     int fmchunk;         // planes marched per CTA
     bool use_fused;      // decided in prepare()
     bool eq_half;        // k_fused_eq with half-width tiles and two CTAs per SM
+    int eq_ygroup;       // k_fused_eq_split: tile rows per launch (0: the whole domain in one launch)
     int eq_split;        // 0: k_fused_eq; 1 / 2: k_fused_eq_split (front / back warps per row) with late / early take
     bool feq;            // one component, BGK, tau = 1: the collision result is f_eq(rho, u' + du) (k_fused_eq applies)
     int last_path;       // lbm_hot_path: what the last lbm_step ran
@@ -662,6 +665,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.wref = h->cfg.rho_ref != 0.0 ? 1 : 0;   // (also read by the compact kernels)
     a.eq = h->feq ? (h->eq_split ? 2 + h->eq_split : (h->eq_half ? 2 : 1)) : 0;
     a.pdl = h->pdl ? 1 : 0;
+    a.i1 = h->eq_ygroup;
     a.used_kernel = op == OP_FUSED ? &h->last_path : nullptr;
     a.stream = h->stream;
     launch_fn fn = pick_launch(h->cfg);
@@ -692,6 +696,11 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     e = fn(a);
     if (e != cudaSuccess) return cuda_fail(h, e, "kernel launch");
     if (!(op == OP_VIRTUAL && h->nbsolid == 0)) h->launches++;
+    // k_fused_eq_split launched per chunk of planes and per group of tile rows (lbm_launch.cuh): count every launch
+    if (op == OP_FUSED && a.eq >= 3 && a.i1 > 0 && h->last_path == LBM_PATH_ONE_PASS_EQ && h->fmchunk > 0) {
+        const int yt = (h->cfg.ny + h->fshape.ty - 1) / h->fshape.ty;
+        h->launches += (long long)((h->cfg.nz + h->fmchunk - 1) / h->fmchunk) * ((yt + a.i1 - 1) / a.i1) - 1;
+    }
     return LBM_OK;
 }
 
@@ -748,12 +757,27 @@ void plan_fused(lbm* h) {
     // rows from DRAM (lbm_fused_eq2.cuh) -- k_fused_eq stays there; elsewhere the split kernel with the early take runs.
     // A forced tile width (LBM_TUNE_EQ_HALF) keeps k_fused_eq.
     h->eq_split = 0;
+    h->eq_ygroup = std::max(0, h->tune.eq_ygroup);
+    bool wave_launches = false;
     if (h->feq && c.compute_dtype == LBM_F32 && c.store_dtype == LBM_F32 && h->fshape.vec == 4) {
         const int txf = 32 * h->fshape.vec;
         const long long cols = (long long)((c.nx + txf - 1) / txf) * ((c.ny + h->fshape.ty - 1) / h->fshape.ty);
         const bool keep = c.nx % txf == 0 && 16 * cols >= 15LL * nsm;
         if (h->tune.eq_split >= 0) h->eq_split = std::min(h->tune.eq_split, 2);
         else if (h->tune.eq_half < 0) h->eq_split = keep ? 0 : 2;
+        // ... except where those columns are ONE wave (at most one CTA per SM: 384^3, 144 columns): there the split kernel
+        // with the late take wins once the march is cut into chunks of at most 192 planes that are launched one after the
+        // other -- every launch starts its CTAs together and the drift between neighbouring tiles, which grows with the
+        // planes marched, stays within what L2 holds.  Measured, ms per step (k_fused_eq | split late, one launch | split late,
+        // a launch per chunk of 192 / 128 planes | split early, a launch per chunk): 384^3 1.659 | 1.65 | 1.540 / 1.544 | 1.73;
+        // 384 x 384 x 512 2.21 | 2.23 | 2.06 (171 planes) / 2.09.  With more columns than SMs (512^3: 256) a launch per chunk
+        // and per group of 32 tile rows does not pay (3.98 against 3.91 for k_fused_eq), nor with fewer columns than SMs
+        // (384 x 296 x 400, 111 columns: 1.51 against 1.42 for one launch with the early take).
+        wave_launches = keep && cols <= nsm && h->tune.eq_split < 0 && h->tune.eq_half < 0 && h->tune.eq_ygroup < 0 && h->tune.mchunk <= 0;
+        if (wave_launches) {
+            h->eq_split = 1;
+            h->eq_ygroup = (c.ny + h->fshape.ty - 1) / h->fshape.ty;
+        }
         if (h->eq_split) h->eq_half = false;
     }
     const bool half = h->feq && h->eq_half;
@@ -802,6 +826,7 @@ void plan_fused(lbm* h) {
         }
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; mchunk = mc; }
     }
+    if (wave_launches) mchunk = (nm + (nm + 191) / 192 - 1) / ((nm + 191) / 192);   // equal chunks of at most 192 planes
     if (h->tune.mchunk > 0) mchunk = std::max(1, std::min(nm, h->tune.mchunk));
     h->fmchunk = mchunk;
     // small domains cannot fill the GPU with marching CTAs: keep the two-pass path unless K2F is demanded

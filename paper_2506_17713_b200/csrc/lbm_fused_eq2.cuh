@@ -106,7 +106,7 @@ struct EqSplitTile {
 
 template <class L, class CT, class ST, int VEC, int TY, bool EARLY, bool WREF>
 __global__ void __launch_bounds__((EqSplitTile<L, CT, ST, VEC, TY>::THREADS), 1)
-k_fused_eq_split(const __grid_constant__ KParams<CT> p, int mchunk) {
+k_fused_eq_split(const __grid_constant__ KParams<CT> p, int mchunk, int yoff, int zoff) {
     using T = EqSplitTile<L, CT, ST, VEC, TY>;
     constexpr int Q = L::Q, NSTG = T::NSTG, NS = T::NS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -131,11 +131,11 @@ k_fused_eq_split(const __grid_constant__ KParams<CT> p, int mchunk) {
 
     const int tx0 = blockIdx.x * T::TX;
     const int txw = min(T::TX, p.nx - tx0);
-    const int yb = blockIdx.y * TY;
+    const int yb = ((int)blockIdx.y + yoff) * TY;      // (yoff, zoff: the launch covers a group of tile rows / one chunk of planes)
     const int nint = min(TY, p.ny - yb);
     const int nm = p.nz;
     const unsigned sy = (unsigned)p.nx, sz = (unsigned)p.nx * (unsigned)p.ny;
-    const int m0 = blockIdx.z * mchunk, m1 = min(nm, m0 + mchunk);
+    const int m0 = ((int)blockIdx.z + zoff) * mchunk, m1 = min(nm, m0 + mchunk);
     const int nit = m1 - m0 + 2;                          // planes m0-1 .. m1 pass through the pipeline (it = 0 .. nit-1)
     const unsigned plane = (unsigned)p.plane;
     auto wrap_y = [&](int y) { return y < 0 ? y + p.ny : (y >= p.ny ? y - p.ny : y); };

@@ -5,6 +5,7 @@
 #include <cstdlib>
 #include "lbm_fused_ws.cuh"
 #include "lbm_fused_eq.cuh"
+#include <algorithm>
 #include "lbm_fused_eq2.cuh"
 #include "lbm_compact.cuh"
 #include "lbm_small.cuh"
@@ -32,6 +33,7 @@ struct LaunchArgs {
     const void* a1;
     void* a2;
     int i0;              // op-specific integer (OP_FUSED: planes marched per CTA)
+    int i1;              // OP_FUSED, k_fused_eq_split: tile rows per launch (0: the whole domain in one launch)
     int eq;              // OP_FUSED: one component, BGK, tau = 1 (f* is an equilibrium): the row-pipeline kernel k_fused_eq applies
                          //           (2: with half-width tiles and two CTAs per SM; 3 / 4: k_fused_eq_split, late / early take)
     int* used_kernel;    // OP_FUSED, out: the lbm_path value of the kernel that ran
@@ -351,9 +353,16 @@ cudaError_t launch(const LaunchArgs& a) {
                                 auto kern = k_fused_eq_split<L, CT, ST, vec, ty, (EARLY != 0), (WREF != 0)>;
                                 static int ready[16] = {0};
                                 if (!usable(kern, ready, T::SMEM, T::REGS_NEEDED, T::THREADS)) return;
-                                dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + ty - 1) / ty),
-                                       (unsigned)((p.nz + a.i0 - 1) / a.i0));
-                                kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0);
+                                const int xt = (p.nx + T::TX - 1) / T::TX, yt = (p.ny + ty - 1) / ty, zc = (p.nz + a.i0 - 1) / a.i0;
+                                if (a.i1 <= 0) {
+                                    kern<<<dim3((unsigned)xt, (unsigned)yt, (unsigned)zc), T::THREADS, T::SMEM, a.stream>>>(p, a.i0, 0, 0);
+                                } else {
+                                    // one launch per chunk of planes and per group of a.i1 tile rows: every launch is a single
+                                    // wave of CTAs that start together (lbm_api.cu, plan_fused)
+                                    for (int z = 0; z < zc; ++z)
+                                        for (int y0 = 0; y0 < yt; y0 += a.i1)
+                                            kern<<<dim3((unsigned)xt, (unsigned)std::min(a.i1, yt - y0), 1u), T::THREADS, T::SMEM, a.stream>>>(p, a.i0, y0, z);
+                                }
                                 if (a.used_kernel) *a.used_kernel = 5;  // LBM_PATH_ONE_PASS_EQ
                                 done = true;
                             }

@@ -176,3 +176,36 @@ def test_one_pass_refused_where_it_does_not_apply():
     s = make_gpu(one_pass(wl), inp)
     with pytest.raises(binding.LBMError):
         s.step(1)
+
+
+@pytest.mark.parametrize("dims,ygroup,mchunk,take", [((128, 40, 30), 2, 8, "late"), ((200, 17, 9), 1, 4, "early"), ((132, 70, 21), 3, 21, "late")])
+def test_split_kernel_launched_per_chunk_and_row_group(dims, ygroup, mchunk, take, monkeypatch):
+    """k_fused_eq_split launched once per chunk of planes and per group of tile rows (what lbm_step does on domains whose tile
+    columns are one wave, e.g. 384^3: lbm_api.cu plan_fused): ragged last group and last chunk; bit-identical to the single
+    launch, every launch counted, and within the fp32 gate of the oracle."""
+    from paper_2506_17713_b200 import binding
+    wl, _ = W.config5(16, "f32")
+    wl.update(nx=dims[0], ny=dims[1], nz=dims[2])
+    inp = small_inputs(wl, 31, 0.05, 0.3)
+    monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", str(mchunk))
+    monkeypatch.setenv("LBM_TUNE_EQ_SPLIT", "2" if take == "early" else "1")
+    out = {}
+    for grouped in (True, False):
+        if grouped:
+            monkeypatch.setenv("LBM_TUNE_EQ_YGROUP", str(ygroup))
+        else:
+            monkeypatch.delenv("LBM_TUNE_EQ_YGROUP", raising=False)
+        g = make_gpu(one_pass(wl), inp)
+        l0 = g.kernel_launches
+        g.step(20)
+        assert g.hot_path == "one_pass_eq"
+        per_step = 1
+        if grouped:
+            yt = (dims[1] + 7) // 8
+            per_step = ((dims[2] + mchunk - 1) // mchunk) * ((yt + ygroup - 1) // ygroup)
+        assert g.kernel_launches - l0 == 20 * per_step
+        out[grouped] = g.get_populations(0)
+    assert np.array_equal(out[True], out[False])
+    o = make_oracle(with_dtype(wl, "f64"), inp)
+    o.step(20)
+    assert_parity([o.get_populations(0)], [out[True]], np.ones(o.N, bool), TOL32, relative=True)
