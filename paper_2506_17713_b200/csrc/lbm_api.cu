@@ -38,6 +38,7 @@ struct Tune {
     int compact = -1;      // LBM_TUNE_COMPACT=0: keep the dense layout where compact mode would apply
     int eq = -1;           // LBM_TUNE_NO_EQ=1 -> 0: k_fused_ws where k_fused_eq would apply
     int eq_half = -1;      // LBM_TUNE_EQ_HALF: force full-width (0) / half-width (1) tiles of k_fused_eq
+    int ws_ty = -1;        // LBM_TUNE_WS_TY: rows per tile of k_fused_ws (fshape.ty or one fewer; -1: chosen per domain)
     int eq_ygroup = -1;    // LBM_TUNE_EQ_YGROUP: k_fused_eq_split launched per chunk of planes and per group of this many tile rows (0: one launch)
     int eq_split = -1;     // LBM_TUNE_EQ_SPLIT: k_fused_eq_split off (0) / on with late (1) / early (2) take; -1: chosen per domain
     bool no_snbr = false;  // LBM_TUNE_NO_SNBR: K1b of the compact mode on the dense rho field
@@ -56,6 +57,7 @@ struct Tune {
         t.eq_half = geti("LBM_TUNE_EQ_HALF", -1);
         t.eq_split = geti("LBM_TUNE_EQ_SPLIT", -1);
         t.eq_ygroup = geti("LBM_TUNE_EQ_YGROUP", -1);
+        t.ws_ty = geti("LBM_TUNE_WS_TY", -1);
         t.no_snbr = std::getenv("LBM_TUNE_NO_SNBR") != nullptr;
         t.no_pdl = std::getenv("LBM_TUNE_NO_PDL") != nullptr;
         t.no_graph = std::getenv("LBM_TUNE_NO_GRAPH") != nullptr;
@@ -85,6 +87,7 @@ struct lbm {
     bool use_fused;      // decided in prepare()
     bool eq_half;        // k_fused_eq with half-width tiles and two CTAs per SM
     int eq_ygroup;       // k_fused_eq_split: tile rows per launch (0: the whole domain in one launch)
+    int ws_ty;           // k_fused_ws: rows per tile chosen by plan_fused (0: fshape.ty)
     int eq_split;        // 0: k_fused_eq; 1 / 2: k_fused_eq_split (front / back warps per row) with late / early take
     bool feq;            // one component, BGK, tau = 1: the collision result is f_eq(rho, u' + du) (k_fused_eq applies)
     int last_path;       // lbm_hot_path: what the last lbm_step ran
@@ -666,6 +669,7 @@ int do_launch(lbm* h, int op, const void* a0, const void* a1, void* a2, int i0, 
     a.eq = h->feq ? (h->eq_split ? 2 + h->eq_split : (h->eq_half ? 2 : 1)) : 0;
     a.pdl = h->pdl ? 1 : 0;
     a.i1 = h->eq_ygroup;
+    a.i2 = h->ws_ty;
     a.used_kernel = op == OP_FUSED ? &h->last_path : nullptr;
     a.stream = h->stream;
     launch_fn fn = pick_launch(h->cfg);
@@ -757,6 +761,7 @@ void plan_fused(lbm* h) {
     // rows from DRAM (lbm_fused_eq2.cuh) -- k_fused_eq stays there; elsewhere the split kernel with the early take runs.
     // A forced tile width (LBM_TUNE_EQ_HALF) keeps k_fused_eq.
     h->eq_split = 0;
+    h->ws_ty = 0;
     h->eq_ygroup = std::max(0, h->tune.eq_ygroup);
     bool wave_launches = false;
     if (h->feq && c.compute_dtype == LBM_F32 && c.store_dtype == LBM_F32 && h->fshape.vec == 4) {
@@ -782,7 +787,27 @@ void plan_fused(lbm* h) {
     }
     const bool half = h->feq && h->eq_half;
     const int tx = 32 * h->fshape.vec / (half ? 2 : 1);
-    const int ty = h->fshape.ty;
+    // k_fused_ws (one component) is bound by the consumers' arithmetic, one warp per tile row: where tiles of one row fewer
+    // give every SM a CTA, the rows per SM and plane shrink with them (256^3, MRT: 64 columns x 2 chunks = 128 CTAs of 8 rows
+    // against 74 x 2 = 148 CTAs of 7).  Chosen by  waves x (planes per chunk + 5) x rows per tile.
+    h->ws_ty = 0;
+    if (!h->feq && c.n_components == 1) {
+        auto best_for = [&](int t) {
+            const long long tl = (long long)((c.nx + tx - 1) / tx) * ((c.ny + t - 1) / t);
+            long long best = -1;
+            for (int nch = 1; nch <= std::max(1, nm / 8); ++nch) {
+                const int mc = (nm + nch - 1) / nch;
+                const long long ctas = tl * ((nm + mc - 1) / mc);
+                const long long cost = ((ctas + nsm - 1) / nsm) * (mc + 5) * t;
+                if (best < 0 || cost < best) best = cost;
+            }
+            return best;
+        };
+        const int t8 = h->fshape.ty, t7 = h->fshape.ty - 1;
+        if (h->tune.ws_ty >= 0) h->ws_ty = h->tune.ws_ty == t7 ? t7 : 0;
+        else if (best_for(t7) < best_for(t8)) h->ws_ty = t7;
+    }
+    const int ty = h->ws_ty > 0 ? h->ws_ty : h->fshape.ty;
     const long long tiles = (long long)((c.nx + tx - 1) / tx) * (h->d == 3 ? (c.ny + ty - 1) / ty : 1);
     // Chunks per column of tiles: every CTA pulls two extra planes and pays a few planes' worth of pipeline fill, and
     // CTAs run in waves of one per SM, so minimise  waves * (planes per chunk + 5)  (measured on 128^3 .. 512^3: the

@@ -34,6 +34,7 @@ struct LaunchArgs {
     void* a2;
     int i0;              // op-specific integer (OP_FUSED: planes marched per CTA)
     int i1;              // OP_FUSED, k_fused_eq_split: tile rows per launch (0: the whole domain in one launch)
+    int i2;              // OP_FUSED, k_fused_ws: rows per tile (0: the default of fused_shape)
     int eq;              // OP_FUSED: one component, BGK, tau = 1 (f* is an equilibrium): the row-pipeline kernel k_fused_eq applies
                          //           (2: with half-width tiles and two CTAs per SM; 3 / 4: k_fused_eq_split, late / early take)
     int* used_kernel;    // OP_FUSED, out: the lbm_path value of the kernel that ran
@@ -320,16 +321,24 @@ cudaError_t launch(const LaunchArgs& a) {
                     constexpr FusedShape fs = fused_shape<L, CT, ST, NC>();
                     if constexpr (fs.vec > 0) {
                         // k_fused_ws: warp-specialised producer / consumer pipeline, two stages of fs.ty rows
-                        auto go_ws = [&](auto WREF) {
-                            using T = WsTile<L, NC, CT, ST, fs.vec, fs.ty, 2>;
-                            auto kern = k_fused_ws<L, NC, CT, ST, C_, fs.vec, fs.ty, 2, (WREF != 0)>;
+                        // (TYW rows per tile: fs.ty, or one fewer where that gives every SM a CTA -- plan_fused, a.i2)
+                        auto go_ws_ty = [&](auto WREF, auto TYW_) {
+                            constexpr int TYW = TYW_;
+                            using T = WsTile<L, NC, CT, ST, fs.vec, TYW, 2>;
+                            auto kern = k_fused_ws<L, NC, CT, ST, C_, fs.vec, TYW, 2, (WREF != 0)>;
                             static int ready[16] = {0};
                             if (!usable(kern, ready, T::SMEM, (long long)T::REG_PROD * T::NPW * 32 + (long long)T::REG_CONS * T::NCW * 32, T::THREADS)) return;
-                            dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + fs.ty - 1) / fs.ty),
+                            dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + TYW - 1) / TYW),
                                    (unsigned)((p.nz + a.i0 - 1) / a.i0));
                             kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0);
                             if (a.used_kernel) *a.used_kernel = 3;  // LBM_PATH_ONE_PASS_WS
                             done = true;
+                        };
+                        auto go_ws = [&](auto WREF) {
+                            if constexpr (NC == 1) {
+                                if (a.i2 == fs.ty - 1) { go_ws_ty(WREF, IC<fs.ty - 1>{}); return; }
+                            }
+                            go_ws_ty(WREF, IC<fs.ty>{});
                         };
                         // k_fused_eq: row pipelines (lbm_fused_eq.cuh); CPS = 2: half-width tiles, two CTAs per SM
                         auto go_eq = [&](auto VEC, auto CPS, auto WREF) {

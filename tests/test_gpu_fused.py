@@ -51,12 +51,14 @@ def run_three(wl, inp, steps, oracle_wl=None):
             [g2.get_populations(k) for k in range(o.nc)], o)
 
 
-@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_eq_split_late", "k_fused_eq_split_early", "k_fused_ws"])
+@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_eq_split_late", "k_fused_eq_split_early", "k_fused_ws",
+                                    "k_fused_ws_7_rows"])
 @pytest.mark.parametrize("dims", [(128, 24, 20), (132, 9, 11), (4, 3, 2), (260, 8, 5), (8, 35, 3)])
 def test_d3q19_fp64_ragged_tiles(dims, kernel, monkeypatch):
     monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "7")   # several marching chunks, ragged last one
-    if kernel == "k_fused_ws":                          # the general kernel where k_fused_eq would apply
+    if kernel.startswith("k_fused_ws"):                 # the general kernel where k_fused_eq would apply
         monkeypatch.setenv("LBM_TUNE_NO_EQ", "1")
+        monkeypatch.setenv("LBM_TUNE_WS_TY", "7" if kernel.endswith("7_rows") else "8")   # rows per tile (plan_fused picks per domain)
     else:
         select_eq_kernel(monkeypatch, kernel)
     wl, _ = W.config5(16, "f64")
@@ -84,10 +86,12 @@ def test_d3q19_fp32_ragged_tiles(dims, kernel, monkeypatch):
     assert_parity(f2, f1, fluid, 2e-6, relative=True)    # same arithmetic as K1 / K2 (fp32: up to contraction of a*b+c)
 
 
-@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_eq_split_late", "k_fused_eq_split_early", "k_fused_ws"])
+@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_eq_split_late", "k_fused_eq_split_early", "k_fused_ws",
+                                    "k_fused_ws_7_rows"])
 def test_config5_fp32_100_steps(kernel, monkeypatch):
-    if kernel == "k_fused_ws":
+    if kernel.startswith("k_fused_ws"):
         monkeypatch.setenv("LBM_TUNE_NO_EQ", "1")
+        monkeypatch.setenv("LBM_TUNE_WS_TY", "7" if kernel.endswith("7_rows") else "8")
     else:
         select_eq_kernel(monkeypatch, kernel)
     wl, inp = W.config5(48, "f32")
@@ -137,7 +141,9 @@ def test_config5_fp16_storage():
     assert_parity(fo, f1, fluid, TOL16, relative=True)
 
 
-def test_config3_mrt_peng_robinson_fp64():
+@pytest.mark.parametrize("rows", [8, 7])
+def test_config3_mrt_peng_robinson_fp64(rows, monkeypatch):
+    monkeypatch.setenv("LBM_TUNE_WS_TY", str(rows))     # rows per tile of k_fused_ws (7 on 256^3: every SM gets a CTA)
     wl, _ = W.config3(20, "f64")
     wl.update(nx=24, ny=19, nz=17)
     inp = small_inputs(wl, 3, 3.9, 4.2)
