@@ -96,7 +96,7 @@ enum lbm_face_kind { LBM_FACE_PERIODIC = 0, LBM_FACE_WALL = 1, LBM_FACE_VELOCITY
  * call reads the environment.  LBM_TUNE_FUSED_MCHUNK=<planes marched per CTA of the one-pass kernels>, LBM_TUNE_NO_EQ (run
  * k_fused_ws where k_fused_eq would apply), LBM_TUNE_EQ_HALF=0|1 (tile width of k_fused_eq), LBM_TUNE_EQ_SPLIT=0|1|2 (k_fused_eq_split off / late / early
  * take), LBM_TUNE_EQ_YGROUP=<tile rows per launch of k_fused_eq_split; with it, one launch per chunk of planes>, LBM_TUNE_WS_TY=7|8 (rows
- * per tile of k_fused_ws, one component), LBM_TUNE_LIST=0|1 and
+ * per tile of k_fused_ws with one component and of k_fused_eq at fp64), LBM_TUNE_LIST=0|1 and
  * LBM_TUNE_COMPACT=0 (list / fluid-compact mode of the two-pass path on masked domains), LBM_TUNE_BRICK="bx,by,bz" (order of
  * the fluid-cell list), LBM_TUNE_NO_SNBR, LBM_TUNE_NO_PDL / LBM_TUNE_NO_GRAPH / LBM_TUNE_NO_COOP (plain launches on small
  * domains), LBM_TUNE_NO_TILE (small 2-D domains on k_steps_coop / graph replay instead of k_steps_tile).  Results never depend on them beyond rounding order (none changes any arithmetic). */

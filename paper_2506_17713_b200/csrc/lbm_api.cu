@@ -791,7 +791,8 @@ void plan_fused(lbm* h) {
     // give every SM a CTA, the rows per SM and plane shrink with them (256^3, MRT: 64 columns x 2 chunks = 128 CTAs of 8 rows
     // against 74 x 2 = 148 CTAs of 7).  Chosen by  waves x (planes per chunk + 5) x rows per tile.
     h->ws_ty = 0;
-    if (!h->feq && c.n_components == 1) {
+    const bool eq64 = h->feq && !h->eq_split && !h->eq_half && c.compute_dtype == LBM_F64;   // k_fused_eq, fp64, full-width tiles
+    if ((!h->feq && c.n_components == 1) || eq64) {
         auto best_for = [&](int t) {
             const long long tl = (long long)((c.nx + tx - 1) / tx) * ((c.ny + t - 1) / t);
             long long best = -1;

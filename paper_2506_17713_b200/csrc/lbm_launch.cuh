@@ -343,15 +343,23 @@ cudaError_t launch(const LaunchArgs& a) {
                         // k_fused_eq: row pipelines (lbm_fused_eq.cuh); CPS = 2: half-width tiles, two CTAs per SM
                         auto go_eq = [&](auto VEC, auto CPS, auto WREF) {
                             if constexpr (NC == 1 && C_ == 0) {
-                                using T = EqTile<L, CT, ST, VEC, fs.ty, CPS>;
-                                auto kern = k_fused_eq<L, CT, ST, VEC, fs.ty, CPS, (WREF != 0)>;
-                                static int ready[16] = {0};
-                                if (!usable(kern, ready, T::SMEM, (long long)T::REG_PROD * T::NPW * 32 + (long long)T::REG_CONS * T::NCW * 32, T::THREADS)) return;
-                                dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + fs.ty - 1) / fs.ty),
-                                       (unsigned)((p.nz + a.i0 - 1) / a.i0));
-                                kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0);
-                                if (a.used_kernel) *a.used_kernel = 5;  // LBM_PATH_ONE_PASS_EQ
-                                done = true;
+                                auto go_ty = [&](auto TYW_) {
+                                    constexpr int TYW = TYW_;
+                                    using T = EqTile<L, CT, ST, VEC, TYW, CPS>;
+                                    auto kern = k_fused_eq<L, CT, ST, VEC, TYW, CPS, (WREF != 0)>;
+                                    static int ready[16] = {0};
+                                    if (!usable(kern, ready, T::SMEM, (long long)T::REG_PROD * T::NPW * 32 + (long long)T::REG_CONS * T::NCW * 32, T::THREADS)) return;
+                                    dim3 g((unsigned)((p.nx + T::TX - 1) / T::TX), (unsigned)((p.ny + TYW - 1) / TYW),
+                                           (unsigned)((p.nz + a.i0 - 1) / a.i0));
+                                    kern<<<g, T::THREADS, T::SMEM, a.stream>>>(p, a.i0);
+                                    if (a.used_kernel) *a.used_kernel = 5;  // LBM_PATH_ONE_PASS_EQ
+                                    done = true;
+                                };
+                                // (7-row tiles where that gives every SM a CTA: full-width tiles, fp64 compute -- plan_fused, a.i2)
+                                if constexpr (sizeof(CT) == 8 && CPS == 1) {
+                                    if (a.i2 == fs.ty - 1) { go_ty(IC<fs.ty - 1>{}); return; }
+                                }
+                                go_ty(IC<fs.ty>{});
                             }
                         };
                         // k_fused_eq_split: front / back warps per row (lbm_fused_eq2.cuh); fp32 compute and storage

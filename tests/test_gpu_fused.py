@@ -51,16 +51,16 @@ def run_three(wl, inp, steps, oracle_wl=None):
             [g2.get_populations(k) for k in range(o.nc)], o)
 
 
-@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_half", "k_fused_eq_split_late", "k_fused_eq_split_early", "k_fused_ws",
-                                    "k_fused_ws_7_rows"])
+@pytest.mark.parametrize("kernel", ["k_fused_eq", "k_fused_eq_7_rows", "k_fused_eq_half", "k_fused_eq_split_late", "k_fused_eq_split_early",
+                                    "k_fused_ws", "k_fused_ws_7_rows"])
 @pytest.mark.parametrize("dims", [(128, 24, 20), (132, 9, 11), (4, 3, 2), (260, 8, 5), (8, 35, 3)])
 def test_d3q19_fp64_ragged_tiles(dims, kernel, monkeypatch):
     monkeypatch.setenv("LBM_TUNE_FUSED_MCHUNK", "7")   # several marching chunks, ragged last one
+    monkeypatch.setenv("LBM_TUNE_WS_TY", "7" if kernel.endswith("7_rows") else "8")   # rows per tile (plan_fused picks per domain)
     if kernel.startswith("k_fused_ws"):                 # the general kernel where k_fused_eq would apply
         monkeypatch.setenv("LBM_TUNE_NO_EQ", "1")
-        monkeypatch.setenv("LBM_TUNE_WS_TY", "7" if kernel.endswith("7_rows") else "8")   # rows per tile (plan_fused picks per domain)
     else:
-        select_eq_kernel(monkeypatch, kernel)
+        select_eq_kernel(monkeypatch, "k_fused_eq" if kernel == "k_fused_eq_7_rows" else kernel)
     wl, _ = W.config5(16, "f64")
     wl.update(nx=dims[0], ny=dims[1], nz=dims[2])
     inp = small_inputs(wl, 21, 0.05, 0.3)
