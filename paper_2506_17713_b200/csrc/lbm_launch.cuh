@@ -103,6 +103,11 @@ cudaError_t launch(const LaunchArgs& a) {
                     constexpr int VW = vec_width<CT, ST, NC>();
                     if constexpr (B != 0) {
                         if (a.list == 2) {
+                            if constexpr (sizeof(ST) == 2) {      // 16-bit storage: two cells per thread (32-bit loads)
+                                if (a.wref) k_moments_c2<L, NC, CT, ST, true><<<grid((p.nfluid + 1) / 2, 256), 256, 0, a.stream>>>(p);
+                                else k_moments_c2<L, NC, CT, ST, false><<<grid((p.nfluid + 1) / 2, 256), 256, 0, a.stream>>>(p);
+                                return;
+                            }
                             if (a.wref) k_moments_c<L, NC, CT, ST, true><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p);
                             else k_moments_c<L, NC, CT, ST, false><<<grid(p.nfluid, 256), 256, 0, a.stream>>>(p);
                             return;
