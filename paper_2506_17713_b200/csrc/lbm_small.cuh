@@ -1,7 +1,9 @@
-// lbm_small.cuh -- the two-pass step of small, launch-bound domains as ONE persistent kernel for n time steps.
+// lbm_small.cuh -- the step of small, launch-bound domains as ONE persistent kernel for n time steps.
 //
-//   k_steps_coop   n x [ K1: rho, psi  |  grid barrier  |  K1b: virtual density  |  grid barrier  |  K2: stream, force,
-//                        collide, boundaries  |  grid barrier ]          (S1..S7; citations as in lbm_hot.cuh)
+//   k_steps_tile   (2-D lattices; configs 1 and 2)  n x [ A: rho, psi on the CTA's tile and a ring around it | B: virtual
+//                  density in shared memory | C: stream, force, collide, boundaries | grid barrier ]   -- below
+//   k_steps_coop   (any lattice)  n x [ K1: rho, psi  |  grid barrier  |  K1b: virtual density  |  grid barrier  |  K2: stream,
+//                  force, collide, boundaries  |  grid barrier ]          (S1..S7; citations as in lbm_hot.cuh)
 //
 // Configs 1 and 2 (0.3 MB and 9.4 MB of state) live in L2 and a step is two or three kernels of a few microseconds: what
 // a step costs there is the launch and drain of each kernel, even when replayed from a CUDA graph with programmatic
@@ -9,8 +11,9 @@
 // keep their cells for all n steps, and meet at a grid barrier between the phases: one atomic per CTA on a monotonic
 // counter, polled with acquire loads.  Everything a phase reads was written by other SMs in the phase before, so global
 // data is loaded with ld.global.cg (L2 only; the read-only path of the other kernels could serve stale L1 lines).
-// Used where every cell gets its own resident thread (config 1: 4.8 -> 4.3 us per step; on config 2, where a thread would
-// take two cells in turn, the separate vectorised kernels stay faster: 11.3 against 14.2 us, so the graph path remains).
+// k_steps_coop is used where every cell gets its own resident thread (config 1: 4.8 -> 4.3 us per step; on config 2, where a
+// thread would take two cells in turn, it loses to the separate vectorised kernels under graph replay: 14.2 against 11.3 us);
+// k_steps_tile needs ONE barrier per step (config 1: 2.2 us, config 2: 6.4 us) and is what lbm_step picks on 2-D lattices.
 // One cell per thread; the arithmetic is that of k_moments_v / k_virtual_density / k_step_v (same device functions, same
 // order of every sum), so the result is bit-identical to the plain launches (tested).
 #pragma once
