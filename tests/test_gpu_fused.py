@@ -215,3 +215,27 @@ def test_split_kernel_launched_per_chunk_and_row_group(dims, ygroup, mchunk, tak
     o = make_oracle(with_dtype(wl, "f64"), inp)
     o.step(20)
     assert_parity([o.get_populations(0)], [out[True]], np.ones(o.N, bool), TOL32, relative=True)
+
+
+@pytest.mark.parametrize("dims,collision", [((128, 1120, 40), "BGK"),    # 140 tile columns: one wave, one chunk
+                                            ((256, 560, 200), "BGK"),    # 140 columns, two launches of 100 planes
+                                            ((256, 256, 40), "MRT"),     # k_fused_ws, 7- against 8-row tiles by the planner
+                                            ((416, 104, 60), "BGK"),     # ragged last x tile: planes per CTA from the play-through
+                                            ((384, 296, 24), "MRT")])
+def test_default_launch_plans_match_the_two_pass_path(dims, collision):
+    """Whatever plan_fused picks for a domain (tile height, planes per CTA, a launch per chunk): the one-pass result equals
+    the two-pass path's to fp32 contraction, on domains large enough to reach those rules (no tuning knob set)."""
+    wl, _ = W.config5(16, "f32")
+    wl.update(nx=dims[0], ny=dims[1], nz=dims[2], collision=collision)
+    if collision == "MRT":
+        wl["mrt_rates"] = [W.mrt_rates("D3Q19", 1.0)]
+    inp = small_inputs(wl, 41, 0.05, 0.3)
+    g1 = make_gpu(wl, inp)
+    g2 = make_gpu(dict(wl, path="two_pass"), inp)
+    g1.step(5)
+    g2.step(5)
+    assert g1.hot_path in ("one_pass_eq", "one_pass_ws"), g1.hot_path
+    assert g2.hot_path == "two_pass"
+    f1, f2 = g1.get_populations(0), g2.get_populations(0)
+    assert np.isfinite(f1).all()
+    assert np.abs(f1 - f2).max() <= 2e-6 * np.abs(f2).max()
